@@ -1,0 +1,202 @@
+"""Seeded synthetic workload generators (shared by the oracle tests, the GPU tests and bench.py).
+
+This module holds NONE of the method's arithmetic: it draws random numbers, rounds them to the
+storage dtype, picks chunk/cache lengths and hands out physical page ids.  The token->slot rule,
+the append and the attention live in `oracle/` (CPU, fp64) and in `csrc/` (CUDA) separately.
+
+Shapes follow BASELINE.json configs 1-5 (B:cfgN) and SURVEY.md §8(d); the paper itself fixes only
+"three latent frames per chunk, 480p" (§7.1, App. B) and the rolling window of
+W in {1,3,7} chunks (§2.1, App. A).  Everything is i.i.d. Gaussian and stands in for
+real AR-DiT activations (the paper's VBench prompts / weights are not available and not needed:
+the path's cost and its correctness depend on shapes only).
+
+Storage dtypes: "f32" arrays are numpy float32; "bf16" arrays are numpy uint16 holding the
+bfloat16 bit pattern (numpy has no bf16), produced by round-to-nearest-even from float32.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+# geometry the configs are built from (B:cfg1, B:cfg2, B:cfg4; "three latent frames")
+FRAMES_PER_CHUNK = 3
+FULL_RES_FRAME_TOKENS = 30 * 52      # 480p latent frame, Wan-1.3B-like (B:cfg2)
+LOW_RES_FRAME_TOKENS = 15 * 26       # low-fidelity stream (B:cfg4)
+TINY_FRAME_TOKENS = 4 * 6            # B:cfg1
+WINDOW_FRAMES = 21                   # B:cfg4 "rolling window capped at 21 latent frames" = 7 chunks (P:568 W=7)
+FULL_RES_CHUNK = FRAMES_PER_CHUNK * FULL_RES_FRAME_TOKENS   # 4680
+LOW_RES_CHUNK = FRAMES_PER_CHUNK * LOW_RES_FRAME_TOKENS     # 1170
+TINY_CHUNK = FRAMES_PER_CHUNK * TINY_FRAME_TOKENS           # 72
+N_LAYERS = 30                        # B:cfg5 "30-layer loop"
+
+
+def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """Round float32 -> bfloat16 (round-to-nearest-even), returned as uint16 bit patterns."""
+    u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
+    rounded = u + np.uint32(0x7FFF) + ((u >> np.uint32(16)) & np.uint32(1))
+    return (rounded >> np.uint32(16)).astype(np.uint16)
+
+
+def bf16_bits_to_f32(b: np.ndarray) -> np.ndarray:
+    """Exact widening of bfloat16 bit patterns to float32 (for handing data to torch / printing)."""
+    return (np.ascontiguousarray(b, dtype=np.uint16).astype(np.uint32) << np.uint32(16)).view(np.float32)
+
+
+@dataclass
+class StreamSpec:
+    """One stream of the batch, in the vocabulary of include/slack.h (slack_stream)."""
+    q_len: int                 # Lq: tokens of the new chunk
+    cache_len: int             # Lc: tokens of earlier chunks held for this stream
+    base: int                  # slot of logical token 0 inside page_table[0]
+    window: int                # Wt: max visible keys including the own chunk; 0 = unlimited
+    sink_len: int              # leading tokens always visible ("sink + local"); 0 in all configs
+    page_table: np.ndarray     # int32 [n_table_pages], logical page -> physical page
+
+    @property
+    def n(self) -> int:
+        return self.cache_len + self.q_len
+
+
+@dataclass
+class Workload:
+    name: str
+    dtype: str                 # "bf16" | "f32"
+    n_heads: int
+    head_dim: int
+    page_size: int
+    n_pages: int
+    scale: float
+    streams: List[StreamSpec]
+    q: np.ndarray              # [sum Lq, H, D] storage dtype
+    k_new: np.ndarray          # [sum Lq, H, D]
+    v_new: np.ndarray          # [sum Lq, H, D]
+    k_prior: List[np.ndarray] = field(default_factory=list)   # per stream [Lc, H, D]
+    v_prior: List[np.ndarray] = field(default_factory=list)
+    seed: int = 0
+
+    @property
+    def storage(self):
+        return np.uint16 if self.dtype == "bf16" else np.float32
+
+    @property
+    def total_q(self) -> int:
+        return int(sum(s.q_len for s in self.streams))
+
+
+def _draw(rng: np.random.Generator, shape, amp: float, dtype: str) -> np.ndarray:
+    x = rng.standard_normal(shape, dtype=np.float32)
+    if amp != 1.0:
+        x *= np.float32(amp)
+    return f32_to_bf16_bits(x) if dtype == "bf16" else x
+
+
+def make_workload(name: str, *, dtype: str, n_heads: int, head_dim: int, page_size: int,
+                  q_lens: Sequence[int], cache_lens: Sequence[int], windows: Sequence[int],
+                  bases: Optional[Sequence[int]] = None, sink_lens: Optional[Sequence[int]] = None,
+                  seed: int = 0, amp: float = 1.0, shuffle_pages: bool = True,
+                  spare_pages: int = 0, scale: Optional[float] = None,
+                  n_pages: Optional[int] = None) -> Workload:
+    """General generator: draws Q/K/V and hands every stream disjoint physical pages.
+
+    Pages come from one global random permutation of the pool (rng seed+7) unless
+    shuffle_pages is False (identity order, B:cfg1).  The pool gets `spare_pages` extra pages that
+    no stream owns (tests fill them with sentinels / NaNs).
+    """
+    n_streams = len(q_lens)
+    bases = list(bases) if bases is not None else [0] * n_streams
+    sink_lens = list(sink_lens) if sink_lens is not None else [0] * n_streams
+    need = [-(-(bases[i] + cache_lens[i] + q_lens[i]) // page_size) for i in range(n_streams)]
+    total = int(sum(need)) + int(spare_pages)
+    if n_pages is None:
+        n_pages = max(total, 1)
+    assert n_pages >= total, "pool too small for the requested streams"
+    prng = np.random.default_rng(seed + 7)
+    order = prng.permutation(n_pages) if shuffle_pages else np.arange(n_pages)
+    rng = np.random.default_rng(seed)
+    streams, k_prior, v_prior = [], [], []
+    at = 0
+    for i in range(n_streams):
+        table = np.ascontiguousarray(order[at:at + need[i]], dtype=np.int32)
+        at += need[i]
+        streams.append(StreamSpec(int(q_lens[i]), int(cache_lens[i]), int(bases[i]), int(windows[i]),
+                                  int(sink_lens[i]), table))
+    tq = int(sum(q_lens))
+    q = _draw(rng, (tq, n_heads, head_dim), amp, dtype)
+    k_new = _draw(rng, (tq, n_heads, head_dim), amp, dtype)
+    v_new = _draw(rng, (tq, n_heads, head_dim), amp, dtype)
+    for i in range(n_streams):
+        k_prior.append(_draw(rng, (int(cache_lens[i]), n_heads, head_dim), amp, dtype))
+        v_prior.append(_draw(rng, (int(cache_lens[i]), n_heads, head_dim), amp, dtype))
+    if scale is None:
+        scale = 1.0 / float(np.sqrt(head_dim))
+    return Workload(name, dtype, n_heads, head_dim, page_size, int(n_pages), float(scale), streams,
+                    q, k_new, v_new, k_prior, v_prior, seed)
+
+
+# ----------------------------------------------------------------------------------------------
+# BASELINE.json configs
+# ----------------------------------------------------------------------------------------------
+
+def config1(seed: int = 0) -> Workload:
+    """B:cfg1 tiny reference: 1 stream, H=2, D=64, fp32, 72 queries, 144 cached, P=16, identity table."""
+    return make_workload("cfg1_tiny_fp32", dtype="f32", n_heads=2, head_dim=64, page_size=16,
+                         q_lens=[TINY_CHUNK], cache_lens=[2 * TINY_CHUNK], windows=[0], seed=seed,
+                         amp=1.0, shuffle_pages=False)
+
+
+def config2(seed: int = 2000, layer: int = 0) -> Workload:
+    """B:cfg2 single Wan-1.3B-like stream: H=12, D=128, bf16, 4680 queries, 4 prior chunks, P=256,
+    92 pages drawn from a shuffled 128-page pool."""
+    return make_workload(f"cfg2_single_stream_L{layer}", dtype="bf16", n_heads=12, head_dim=128,
+                         page_size=256, q_lens=[FULL_RES_CHUNK], cache_lens=[4 * FULL_RES_CHUNK],
+                         windows=[0], seed=seed + layer, amp=0.5, n_pages=128)
+
+
+def config3(seed: int = 3000, layer: int = 0) -> Workload:
+    """B:cfg3 ragged batch of 8 streams, prior chunks ~ U{0..6}."""
+    priors = np.random.default_rng(seed + 7).integers(0, 7, size=8)
+    return make_workload(f"cfg3_ragged8_L{layer}", dtype="bf16", n_heads=12, head_dim=128, page_size=256,
+                         q_lens=[FULL_RES_CHUNK] * 8, cache_lens=[int(p) * FULL_RES_CHUNK for p in priors],
+                         windows=[0] * 8, seed=seed + layer, amp=0.5, spare_pages=16)
+
+
+def config4(seed: int = 4000, layer: int = 0) -> Workload:
+    """B:cfg4 mixed fidelity: 8 full-res + 8 low-res streams, 21-frame rolling window, priors ~ U{0..7}
+    (reading A3: 7 priors leaves the oldest chunk resident but outside the window)."""
+    priors = np.random.default_rng(seed + 7).integers(0, 8, size=16)
+    q_lens = [FULL_RES_CHUNK] * 8 + [LOW_RES_CHUNK] * 8
+    windows = [WINDOW_FRAMES * FULL_RES_FRAME_TOKENS] * 8 + [WINDOW_FRAMES * LOW_RES_FRAME_TOKENS] * 8
+    return make_workload(f"cfg4_mixed16_L{layer}", dtype="bf16", n_heads=12, head_dim=128, page_size=256,
+                         q_lens=q_lens, cache_lens=[int(p) * q for p, q in zip(priors, q_lens)],
+                         windows=windows, seed=seed + layer, amp=0.5, spare_pages=16)
+
+
+def config5(kv_chunks: int = 7, seed: int = 5000, layer: int = 0) -> Workload:
+    """B:cfg5 long-cache point: 4 streams, Lk = kv_chunks*4680 (1..7), full 21-frame window."""
+    assert 1 <= kv_chunks <= 7
+    return make_workload(f"cfg5_long4_k{kv_chunks}_L{layer}", dtype="bf16", n_heads=12, head_dim=128,
+                         page_size=256, q_lens=[FULL_RES_CHUNK] * 4,
+                         cache_lens=[(kv_chunks - 1) * FULL_RES_CHUNK] * 4,
+                         windows=[WINDOW_FRAMES * FULL_RES_FRAME_TOKENS] * 4, seed=seed + layer, amp=0.5)
+
+
+def config5b(seed: int = 5500, n_streams: int = 64) -> Workload:
+    """Supplementary decode-like case: 64 streams, 72-query chunks, 8190 keys."""
+    return make_workload("cfg5b_decode_like", dtype="bf16", n_heads=12, head_dim=128, page_size=256,
+                         q_lens=[TINY_CHUNK] * n_streams, cache_lens=[8190 - TINY_CHUNK] * n_streams,
+                         windows=[0] * n_streams, seed=seed, amp=0.5)
+
+
+def small_ragged(seed: int = 11, dtype: str = "bf16", n_heads: int = 2, head_dim: int = 128,
+                 page_size: int = 128, amp: float = 0.5) -> Workload:
+    """Parity-test sized ragged batch the oracle finishes in seconds: spans several 128-row tiles with
+    ragged tails, a Lq=1 stream, a Lq=129 stream, an empty cache, a mid-page base and a clipped window."""
+    q_lens = [300, 1, 129, 72, 257, 0, 128]
+    cache_lens = [517, 700, 0, 1000, 255, 64, 384]
+    windows = [0, 0, 0, 600, 400, 0, 0]
+    bases = [0, 5, 127 % page_size, 77 % page_size, 1, 0, 0]
+    return make_workload(f"small_ragged_{dtype}", dtype=dtype, n_heads=n_heads, head_dim=head_dim,
+                         page_size=page_size, q_lens=q_lens, cache_lens=cache_lens, windows=windows,
+                         bases=bases, seed=seed, amp=amp, spare_pages=3)
