@@ -1,0 +1,164 @@
+/* slack.h — C ABI of libslack: ragged, batched chunk attention over per-stream paged KV caches (B200, sm_100a).
+ *
+ * What the calls compute, and where that is defined
+ * -------------------------------------------------
+ * An AR-DiT generates a stream chunk by chunk; each chunk's tokens attend to the cached K/V of the stream's
+ * earlier chunks and the finished chunk's K/V is appended to a rolling KV cache (§1, §2.1).
+ * The cache is bounded by a rolling window over the most recent chunks (§2.1, knob (3) P:88, W in {1,3,7}
+ * chunks P:568 App. A) and lives in a per-worker PAGED pool addressed through a logical page table
+ * (§3.2, §4.4).  Several streams' caches are co-resident in one GPU's pool (§4.1).
+ * Everything the paper leaves open (mask inside the chunk, what the window counts, pool layout, scale,
+ * append-then-attend, co-batching) follows BASELINE.json north_star/configs as read in DESIGN.md "Readings".
+ *
+ * For stream s, head h, with Lq = q_len, Lc = cache_len, n = Lc + Lq, Wt = window:
+ *     lo      = (Wt > 0) ? max(0, n - Wt) : 0
+ *     visible = { t : lo <= t < n }                        (own chunk included; bidirectional inside the chunk)
+ *     out_i   = sum_{t in visible} softmax_t(scale * <q_i, k_t>) * v_t        for every query row i of the chunk
+ *     lse_i   = ln sum_{t in visible} exp(scale * <q_i, k_t>)
+ *
+ * Token -> slot rule (the single source of truth for "page-table indexing"):
+ *     logical token t of a stream lives at physical page  page_table[(base + t) / page_size],
+ *     slot (base + t) % page_size, i.e. element offset ((page * n_heads + h) * page_size + slot) * head_dim + d
+ *     of a pool tensor laid out [n_pages][n_heads][page_size][head_dim] (head_dim contiguous).
+ *
+ * Ownership: every device buffer (pools, q, k_new, v_new, out, lse, workspace) is CALLER-owned.  The library owns
+ * only the context, plans and their small device-side tables.  Host descriptor arrays (slack_stream, page tables)
+ * are read during the call only.  All device work is enqueued on the caller's CUDA stream; no call synchronises the
+ * device except slack_plan (one small upload, synchronous) and slack_destroy / slack_plan_destroy.
+ * Errors: every call returns a slack_status and never aborts, throws or prints; slack_last_error() gives a text.
+ * A context is not thread-safe; plans are immutable after creation.
+ * There is NO CPU fallback: without a CUDA device only host-only contexts (device = -1) exist, and they can plan
+ * (for inspection) but every data-path call on them returns SLACK_ECUDA.
+ */
+#ifndef SLACK_H_
+#define SLACK_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SLACK_ABI_VERSION 1
+
+typedef enum {
+  SLACK_OK = 0,
+  SLACK_EINVAL = 1,       /* malformed descriptors: negative lengths, base >= page_size, short page table, page id out of
+                             range, a physical page owned twice in the batch, misaligned (<16 B) pointer, NULL argument */
+  SLACK_EUNSUPPORTED = 2, /* valid but not built: sink_len != 0, head_dim not in {64,128}, page_size not a power of two >= 16 */
+  SLACK_ENOMEM = 3,       /* host or device allocation failed, or workspace_bytes too small */
+  SLACK_ECUDA = 4,        /* a CUDA runtime/driver call failed, or the context has no device */
+  SLACK_ESTALE_PLAN = 5   /* plan does not match the pool shape / dtype passed with it */
+} slack_status;
+
+typedef enum { SLACK_BF16 = 0, SLACK_F32 = 1 } slack_dtype;
+
+typedef struct slack_ctx slack_ctx;   /* opaque */
+typedef struct slack_plan_s slack_plan_t; /* opaque */
+
+/* One layer's pool ("paged pool", "logical page table").  k_pool / v_pool: DEVICE pointers, each
+ * [n_pages][n_heads][page_size][head_dim] of `dtype`, head_dim contiguous, 16-byte aligned (128-byte for bf16 with
+ * head_dim 128: required by TMA).  slack_plan reads only the shape fields (pointers may be NULL there). */
+typedef struct {
+  void *k_pool;
+  void *v_pool;
+  int32_t n_pages, n_heads, head_dim, page_size;
+  int32_t dtype; /* slack_dtype */
+} slack_pool;
+
+/* One stream of the batch; HOST memory. */
+typedef struct {
+  int32_t q_len;             /* Lq: tokens of the new chunk (0 = legal no-op)                                   */
+  int32_t cache_len;         /* Lc: tokens of earlier chunks held for this stream                               */
+  int32_t base;              /* slot of logical token 0 inside page_table[0]; 0 <= base < page_size             */
+  int32_t window;            /* Wt: max visible keys INCLUDING the own chunk; 0 = unlimited              */
+  int32_t sink_len;          /* reserved ("sink + local"); must be 0, else SLACK_EUNSUPPORTED             */
+  int32_t n_table_pages;     /* >= ceil((base + Lc + Lq) / page_size)                                           */
+  const int32_t *page_table; /* HOST: logical page -> physical page id in [0, n_pages)                          */
+} slack_stream;
+
+/* Planner options; NULL = all defaults. */
+typedef struct {
+  int32_t sm_count;     /* CTAs the attention kernel is planned for; 0 = the device's SM count (148 on B200;
+                           host-only contexts default to 148)                                                   */
+  int32_t force_splits; /* 0 = automatic split-KV; k >= 1 = cut every (stream, head, q-tile) item's key range into
+                           exactly min(k, #kv tiles) parts (1 = never split)                                     */
+  int32_t force_simt;   /* 1 = plan for the fp32-accumulating SIMT validation kernel even where the tensor-core path
+                           applies (debug / cross-check); f32 pools always use it                                */
+  int32_t reserved;
+} slack_plan_opts;
+
+/* One unit of attention work as planned (inspection only; see slack_plan_get_items). Key tiles are 128 pool slots,
+ * anchored to page slots: tile index T covers positions [128*T, 128*T+128) of the stream's position space
+ * pos = base + t.  */
+typedef struct {
+  int32_t stream;        /* index into the batch                                                                 */
+  int32_t head;
+  int32_t q_row0;        /* first query row (global row of the ragged concat)                                    */
+  int32_t q_rows;        /* valid rows, 1..256 (two 128-row MMA tiles)                                           */
+  int32_t kv_tile_begin; /* [begin, end) in position-tile units                                                  */
+  int32_t kv_tile_end;
+  int32_t pos_lo;        /* visible positions [pos_lo, pos_hi) = [base + lo, base + n)                           */
+  int32_t pos_hi;
+  int32_t partial_slot;  /* -1: writes `out` directly; >= 0: writes workspace slot (split-KV), combined afterwards */
+  int32_t cta;           /* CTA (0..sm_count-1) whose queue holds this item                                      */
+} slack_work_item;
+
+/* ---- context ------------------------------------------------------------------------------------------------ */
+/* device >= 0: CUDA device ordinal.  device = -1: host-only context (planning/inspection, no CUDA call is made).  */
+slack_status slack_create(slack_ctx **ctx, int device);
+void slack_destroy(slack_ctx *ctx);
+const char *slack_last_error(const slack_ctx *ctx); /* ctx-owned string, valid until the next call on ctx */
+int32_t slack_abi_version(void);
+
+/* ---- A1: KV append ("appended to a rolling KV cache") -------------------------------------------------- */
+/* Copies k_new / v_new (DEVICE, ragged concat [sum Lq][n_heads][head_dim] in stream order, 16-byte aligned) into
+ * the slots of logical tokens [Lc, Lc+Lq) of every stream.  Pure copy: bit-exact, touches no other byte.
+ * Re-appending at the same position overwrites (a later denoising step of the same chunk).  Asynchronous on
+ * `cuda_stream` (a cudaStream_t; NULL = default stream).  The descriptor tables are staged through a ctx-owned
+ * pinned buffer; for the per-layer hot loop use slack_kv_append_planned, which re-uses the plan's device tables. */
+slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_streams, const slack_stream *streams,
+                             const void *k_new, const void *v_new, void *cuda_stream);
+slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool,
+                                     const void *k_new, const void *v_new, void *cuda_stream);
+
+/* ---- A2: plan (host) ---------------------------------------------------------------------------------------- */
+/* Validates the batch, cuts it into (stream, head, q-tile, kv-tile-range) work items, balances them over the SMs
+ * (split-KV where a key range is cut), builds the combine list and uploads the tables (one synchronous copy).  The
+ * plan depends only on (q_len, cache_len, base, window, page_table, n_heads, head_dim, page_size, dtype): it is valid
+ * for every layer and denoising step of the chunk batch (same page ids in every layer's pool). */
+slack_status slack_plan(slack_ctx *ctx, const slack_pool *pool_shape, int32_t n_streams,
+                        const slack_stream *streams, const slack_plan_opts *opts, slack_plan_t **plan);
+void slack_plan_destroy(slack_plan_t *plan);
+size_t slack_plan_workspace_bytes(const slack_plan_t *plan); /* device bytes slack_chunk_attention needs (may be 0) */
+int32_t slack_plan_num_items(const slack_plan_t *plan);
+int32_t slack_plan_num_partial_slots(const slack_plan_t *plan);
+int32_t slack_plan_kernel_kind(const slack_plan_t *plan);    /* 0 = tcgen05 tensor-core kernel, 1 = SIMT kernel */
+/* Copies up to `capacity` planned items (in queue order) to `items`; returns how many were written. */
+int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, int32_t capacity);
+
+/* ---- A3 + A4: chunk attention and split-KV combine ------------------------------------------------------------ */
+/* Precondition: the own chunk's K/V is already appended (pool holds logical tokens [0, Lc+Lq) of every stream).
+ * q, out: DEVICE [sum Lq][n_heads][head_dim] of the pool dtype (16-byte aligned; 128-byte for the bf16 path);
+ * lse: optional DEVICE fp32 [n_heads][sum Lq] (natural log), may be NULL; workspace: DEVICE, >=
+ * slack_plan_workspace_bytes(plan) bytes, 16-byte aligned, may be NULL when that is 0.  Asynchronous on cuda_stream. */
+slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q,
+                                   void *out, float *lse, float scale, void *workspace, size_t workspace_bytes,
+                                   void *cuda_stream);
+
+/* Number of kernels the last slack_chunk_attention / slack_kv_append call on this ctx launched (bench bookkeeping). */
+int32_t slack_last_launch_count(const slack_ctx *ctx);
+
+/* ---- diagnostics (never on the data path) ---------------------------------------------------------------------- */
+/* key 0: `value` = DEVICE pointer to a [2][128][128] fp32 buffer that receives the first two S = QK^T tiles computed by
+ * CTA 0 of the next tensor-core launches (NULL switches the dump off). */
+slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value);
+/* Every in-kernel barrier wait is bounded; a wait that times out records {0xDEAD, block<<32|thread, tag<<32|parity, 0}
+ * in host-mapped memory and traps the launch (reported as SLACK_ECUDA by the next call).  This reads that record. */
+slack_status slack_debug_timeout(slack_ctx *ctx, uint64_t out[4]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLACK_H_ */

@@ -1,0 +1,258 @@
+"""ctypes binding of libslack.so (include/slack.h) — argument marshalling only.
+
+Every step of the hot path (append, plan, attention, combine) runs inside the library; this module converts torch
+tensors / StreamSpec-like objects to the plain pointers and structs of the C ABI and raises on any non-OK status.
+It never falls back to anything: a missing library raises ImportError-like RuntimeError at load time.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_PKG_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG_DIR, "libslack.so")
+
+SLACK_OK, SLACK_EINVAL, SLACK_EUNSUPPORTED, SLACK_ENOMEM, SLACK_ECUDA, SLACK_ESTALE_PLAN = range(6)
+STATUS_NAMES = ["SLACK_OK", "SLACK_EINVAL", "SLACK_EUNSUPPORTED", "SLACK_ENOMEM", "SLACK_ECUDA", "SLACK_ESTALE_PLAN"]
+SLACK_BF16, SLACK_F32 = 0, 1
+DTYPES = {"bf16": SLACK_BF16, "f32": SLACK_F32}
+
+
+class SlackError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < 6 else status}: {message}")
+        self.status = status
+
+
+class CPool(C.Structure):
+    _fields_ = [("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("n_pages", C.c_int32), ("n_heads", C.c_int32),
+                ("head_dim", C.c_int32), ("page_size", C.c_int32), ("dtype", C.c_int32)]
+
+
+class CStream(C.Structure):
+    _fields_ = [("q_len", C.c_int32), ("cache_len", C.c_int32), ("base", C.c_int32), ("window", C.c_int32),
+                ("sink_len", C.c_int32), ("n_table_pages", C.c_int32), ("page_table", C.POINTER(C.c_int32))]
+
+
+class CPlanOpts(C.Structure):
+    _fields_ = [("sm_count", C.c_int32), ("force_splits", C.c_int32), ("force_simt", C.c_int32), ("reserved", C.c_int32)]
+
+
+class CWorkItem(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("stream", "head", "q_row0", "q_rows", "kv_tile_begin", "kv_tile_end",
+                                         "pos_lo", "pos_hi", "partial_slot", "cta")]
+
+
+# every symbol include/slack.h declares: name -> (restype, argtypes)
+_VP = C.c_void_p
+SYMBOLS = {
+    "slack_abi_version": (C.c_int32, []),
+    "slack_create": (C.c_int, [C.POINTER(_VP), C.c_int]),
+    "slack_destroy": (None, [_VP]),
+    "slack_last_error": (C.c_char_p, [_VP]),
+    "slack_last_launch_count": (C.c_int32, [_VP]),
+    "slack_kv_append": (C.c_int, [_VP, C.POINTER(CPool), C.c_int32, C.POINTER(CStream), _VP, _VP, _VP]),
+    "slack_kv_append_planned": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP]),
+    "slack_plan": (C.c_int, [_VP, C.POINTER(CPool), C.c_int32, C.POINTER(CStream), C.POINTER(CPlanOpts), C.POINTER(_VP)]),
+    "slack_plan_destroy": (None, [_VP]),
+    "slack_plan_workspace_bytes": (C.c_size_t, [_VP]),
+    "slack_plan_num_items": (C.c_int32, [_VP]),
+    "slack_plan_num_partial_slots": (C.c_int32, [_VP]),
+    "slack_plan_kernel_kind": (C.c_int32, [_VP]),
+    "slack_plan_get_items": (C.c_int32, [_VP, C.POINTER(CWorkItem), C.c_int32]),
+    "slack_chunk_attention": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP, C.c_size_t, _VP]),
+    "slack_debug_set": (C.c_int, [_VP, C.c_int32, _VP]),
+    "slack_debug_timeout": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
+}
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen libslack.so and type its symbols; raises if the library has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_15319_b200.build` "
+                               "(there is no fallback path)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _stream_array(streams: Sequence):
+    """slack_stream[] from StreamSpec-like objects (q_len, cache_len, base, window, sink_len, page_table)."""
+    arr = (CStream * max(len(streams), 1))()
+    keep = []
+    for i, s in enumerate(streams):
+        table = np.ascontiguousarray(s.page_table, dtype=np.int32)
+        keep.append(table)
+        arr[i] = CStream(int(s.q_len), int(s.cache_len), int(s.base), int(s.window), int(getattr(s, "sink_len", 0)),
+                         int(table.size), table.ctypes.data_as(C.POINTER(C.c_int32)))
+    return arr, keep
+
+
+def _ptr(t) -> Optional[int]:
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    return t.data_ptr()
+
+
+def _cuda_stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        if torch.cuda.is_available():
+            return torch.cuda.current_stream().cuda_stream or None
+        return None
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None
+
+
+class Pool:
+    """One layer's K/V pool: torch tensors [n_pages, H, P, D] (bf16 or f32), caller-owned."""
+
+    def __init__(self, k_pool, v_pool, n_pages: int, n_heads: int, head_dim: int, page_size: int, dtype: str):
+        self.k_pool, self.v_pool = k_pool, v_pool
+        self.c = CPool(_ptr(k_pool), _ptr(v_pool), n_pages, n_heads, head_dim, page_size, DTYPES[dtype])
+
+    @classmethod
+    def shape_only(cls, n_pages, n_heads, head_dim, page_size, dtype):
+        return cls(None, None, n_pages, n_heads, head_dim, page_size, dtype)
+
+
+class Plan:
+    def __init__(self, ctx: "Context", handle: int):
+        self.ctx, self.handle = ctx, handle
+
+    def close(self):
+        if self.handle:
+            load().slack_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(load().slack_plan_workspace_bytes(self.handle))
+
+    @property
+    def num_items(self) -> int:
+        return int(load().slack_plan_num_items(self.handle))
+
+    @property
+    def num_partial_slots(self) -> int:
+        return int(load().slack_plan_num_partial_slots(self.handle))
+
+    @property
+    def kernel_kind(self) -> int:
+        return int(load().slack_plan_kernel_kind(self.handle))
+
+    def items(self):
+        n = self.num_items
+        buf = (CWorkItem * max(n, 1))()
+        got = load().slack_plan_get_items(self.handle, buf, n)
+        names = [f[0] for f in CWorkItem._fields_]
+        return [{k: int(getattr(buf[i], k)) for k in names} for i in range(got)]
+
+
+class Context:
+    """slack_ctx wrapper. device=-1 gives a host-only context (planning / inspection only)."""
+
+    def __init__(self, device: int = 0):
+        self.lib = load()
+        h = _VP()
+        st = self.lib.slack_create(C.byref(h), device)
+        if st != SLACK_OK:
+            raise SlackError(st, f"slack_create(device={device}) failed")
+        self.handle = h.value
+        self.device = device
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.slack_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != SLACK_OK:
+            raise SlackError(st, self.lib.slack_last_error(self.handle).decode())
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(self.lib.slack_last_launch_count(self.handle))
+
+    # --- the three calls of the boundary, same names as the C ABI ---------------------------------------------------
+    def slack_plan(self, pool: Pool, streams: Sequence, sm_count: int = 0, force_splits: int = 0,
+                   force_simt: int = 0) -> Plan:
+        arr, keep = _stream_array(streams)
+        opts = CPlanOpts(sm_count, force_splits, force_simt, 0)
+        h = _VP()
+        self._check(self.lib.slack_plan(self.handle, C.byref(pool.c), len(streams), arr, C.byref(opts), C.byref(h)))
+        del keep
+        return Plan(self, h.value)
+
+    def slack_kv_append(self, pool: Pool, streams: Sequence, k_new, v_new, stream=None) -> None:
+        arr, keep = _stream_array(streams)
+        self._check(self.lib.slack_kv_append(self.handle, C.byref(pool.c), len(streams), arr, _ptr(k_new), _ptr(v_new),
+                                             _cuda_stream(stream)))
+        del keep
+
+    def slack_kv_append_planned(self, plan: Plan, pool: Pool, k_new, v_new, stream=None) -> None:
+        self._check(self.lib.slack_kv_append_planned(self.handle, plan.handle, C.byref(pool.c), _ptr(k_new), _ptr(v_new),
+                                                     _cuda_stream(stream)))
+
+    def slack_chunk_attention(self, plan: Plan, pool: Pool, q, out, scale: float, lse=None, workspace=None,
+                              stream=None) -> None:
+        ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+        self._check(self.lib.slack_chunk_attention(self.handle, plan.handle, C.byref(pool.c), _ptr(q), _ptr(out), _ptr(lse),
+                                                   C.c_float(scale), _ptr(workspace), ws_bytes, _cuda_stream(stream)))
+
+    # --- diagnostics --------------------------------------------------------------------------------------------------
+    def debug_set_s_dump(self, tensor) -> None:
+        self._check(self.lib.slack_debug_set(self.handle, 0, _ptr(tensor)))
+
+    def debug_timeout(self):
+        buf = (C.c_uint64 * 4)()
+        self.lib.slack_debug_timeout(self.handle, buf)
+        return [int(x) for x in buf]
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# storage helpers (numpy bit patterns <-> torch tensors); no arithmetic
+# ---------------------------------------------------------------------------------------------------------------------
+
+def to_torch(arr: np.ndarray, dtype: str, device="cpu", pin: bool = False):
+    """numpy storage array (uint16 bf16 bit patterns, or float32) -> torch tensor of the same bits."""
+    import torch
+    a = np.ascontiguousarray(arr)
+    t = torch.from_numpy(a.view(np.int16)).view(torch.bfloat16) if dtype == "bf16" else torch.from_numpy(a)
+    if pin:
+        t = t.pin_memory()
+    return t.to(device) if str(device) != "cpu" else t
+
+
+def to_numpy(t, dtype: str) -> np.ndarray:
+    """torch tensor -> numpy storage array (uint16 bit patterns for bf16)."""
+    import torch
+    t = t.detach().cpu().contiguous()
+    if dtype == "bf16":
+        return t.view(torch.int16).numpy().view(np.uint16)
+    return t.numpy()

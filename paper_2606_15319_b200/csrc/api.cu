@@ -1,0 +1,418 @@
+// api.cu — the C ABI of include/slack.h: context, plan objects, argument checks, TMA descriptors, kernel launches.
+// No arithmetic of the method lives here; see append.cu / attn_tc.cu / attn_simt.cu / combine.cu.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "kernels.h"
+#include "slack_internal.h"
+
+using namespace slack;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct slack_ctx {
+  int device = -1;
+  int sm_count = 148;
+  std::string err;
+  int last_launches = 0;
+  EncodeTiledFn encode = nullptr;
+  bool tc_configured = false;
+  // staging for slack_kv_append (descriptor tables of an unplanned append)
+  void *h_stage = nullptr;
+  void *d_stage = nullptr;
+  size_t stage_cap = 0;
+  cudaEvent_t stage_ev = nullptr;
+  bool stage_pending = false;
+  // diagnostics
+  unsigned long long *h_dbg = nullptr; // mapped pinned, 4 words, survives a trapped launch
+  unsigned long long *d_dbg = nullptr;
+  float *dbg_s = nullptr;
+};
+
+struct slack_plan_s {
+  slack_ctx *ctx = nullptr;
+  HostPlan hp;
+  int max_q_len = 0;
+  void *d_blob = nullptr; // one allocation holding all tables
+  DevStream *d_streams = nullptr;
+  int32_t *d_page_tables = nullptr;
+  DevItem *d_items = nullptr;
+  int32_t *d_cta_begin = nullptr;
+  DevCombine *d_combines = nullptr;
+};
+
+namespace {
+
+slack_status set_err(slack_ctx *ctx, slack_status st, const std::string &msg) {
+  if (ctx) ctx->err = msg;
+  return st;
+}
+slack_status cuda_err(slack_ctx *ctx, cudaError_t e, const char *what) {
+  char buf[256];
+  snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+  return set_err(ctx, SLACK_ECUDA, buf);
+}
+#define SLACK_CUDA(ctx, call)                                  \
+  do {                                                         \
+    cudaError_t e__ = (call);                                  \
+    if (e__ != cudaSuccess) return cuda_err(ctx, e__, #call);  \
+  } while (0)
+
+bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+slack_status ensure_device(slack_ctx *ctx) {
+  if (!ctx) return SLACK_EINVAL;
+  if (ctx->device < 0) return set_err(ctx, SLACK_ECUDA, "host-only context: no CUDA device (there is no CPU fallback)");
+  int cur = -1;
+  SLACK_CUDA(ctx, cudaGetDevice(&cur));
+  if (cur != ctx->device) SLACK_CUDA(ctx, cudaSetDevice(ctx->device));
+  return SLACK_OK;
+}
+
+slack_status check_pool(slack_ctx *ctx, const slack_pool *pool, const HostPlan *hp) {
+  if (!pool || !pool->k_pool || !pool->v_pool) return set_err(ctx, SLACK_EINVAL, "pool or pool pointers NULL");
+  if (!aligned(pool->k_pool, 16) || !aligned(pool->v_pool, 16)) return set_err(ctx, SLACK_EINVAL, "pool pointers must be 16-byte aligned");
+  if (hp && (pool->n_pages != hp->n_pages || pool->n_heads != hp->n_heads || pool->head_dim != hp->head_dim ||
+             pool->page_size != hp->page_size || pool->dtype != hp->dtype))
+    return set_err(ctx, SLACK_ESTALE_PLAN, "plan was made for a different pool shape / dtype");
+  return SLACK_OK;
+}
+
+slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t cols, uint64_t rows) {
+  const cuuint64_t dims[2] = {cols, rows};
+  const cuuint64_t strides[1] = {cols * 2};
+  const cuuint32_t box[2] = {64, 128};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    char buf[128];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    return set_err(ctx, SLACK_ECUDA, buf);
+  }
+  return SLACK_OK;
+}
+
+int elem_bytes(int dtype) { return dtype == SLACK_BF16 ? 2 : 4; }
+
+} // namespace
+
+extern "C" {
+
+int32_t slack_abi_version(void) { return SLACK_ABI_VERSION; }
+
+slack_status slack_create(slack_ctx **out, int device) {
+  if (!out) return SLACK_EINVAL;
+  *out = nullptr;
+  slack_ctx *ctx = new (std::nothrow) slack_ctx();
+  if (!ctx) return SLACK_ENOMEM;
+  ctx->device = device;
+  if (device >= 0) {
+    cudaError_t e = cudaSetDevice(device);
+    int sm = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) {
+      ctx->sm_count = sm;
+      void *fn = nullptr;
+      cudaDriverEntryPointQueryResult qres;
+      e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+      if (e == cudaSuccess && qres == cudaDriverEntryPointSuccess) ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->stage_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) {
+      e = cudaHostAlloc(reinterpret_cast<void **>(&ctx->h_dbg), 4 * sizeof(unsigned long long), cudaHostAllocMapped);
+      if (e == cudaSuccess) {
+        memset(ctx->h_dbg, 0, 4 * sizeof(unsigned long long));
+        e = cudaHostGetDevicePointer(reinterpret_cast<void **>(&ctx->d_dbg), ctx->h_dbg, 0);
+      }
+    }
+    if (e != cudaSuccess) {
+      delete ctx;
+      return SLACK_ECUDA;
+    }
+  }
+  *out = ctx;
+  return SLACK_OK;
+}
+
+void slack_destroy(slack_ctx *ctx) {
+  if (!ctx) return;
+  if (ctx->device >= 0) {
+    cudaSetDevice(ctx->device);
+    if (ctx->stage_pending) cudaEventSynchronize(ctx->stage_ev);
+    if (ctx->stage_ev) cudaEventDestroy(ctx->stage_ev);
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->d_stage) cudaFree(ctx->d_stage);
+    if (ctx->h_dbg) cudaFreeHost(ctx->h_dbg);
+  }
+  delete ctx;
+}
+
+const char *slack_last_error(const slack_ctx *ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
+int32_t slack_last_launch_count(const slack_ctx *ctx) { return ctx ? ctx->last_launches : 0; }
+
+/* diagnostics (not part of the data path): key 0 = device pointer of a [2][128][128] fp32 buffer receiving the first
+ * S tiles of CTA 0 (NULL disables); slack_debug_timeout copies the 4-word time-out record of the last trapped launch. */
+slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value) {
+  if (!ctx) return SLACK_EINVAL;
+  if (key == 0) {
+    ctx->dbg_s = reinterpret_cast<float *>(value);
+    return SLACK_OK;
+  }
+  return set_err(ctx, SLACK_EINVAL, "unknown debug key");
+}
+slack_status slack_debug_timeout(slack_ctx *ctx, uint64_t out[4]) {
+  if (!ctx || !out) return SLACK_EINVAL;
+  for (int i = 0; i < 4; ++i) out[i] = ctx->h_dbg ? ctx->h_dbg[i] : 0;
+  return SLACK_OK;
+}
+
+/* ------------------------------------------------------------------------------------------------ plan */
+slack_status slack_plan(slack_ctx *ctx, const slack_pool *pool_shape, int32_t n_streams, const slack_stream *streams,
+                        const slack_plan_opts *opts, slack_plan_t **plan_out) {
+  if (!ctx) return SLACK_EINVAL;
+  if (!pool_shape || !plan_out) return set_err(ctx, SLACK_EINVAL, "pool_shape or plan NULL");
+  *plan_out = nullptr;
+  slack_plan_opts o{};
+  if (opts) o = *opts;
+  slack_plan_s *pl = new (std::nothrow) slack_plan_s();
+  if (!pl) return set_err(ctx, SLACK_ENOMEM, "out of host memory");
+  pl->ctx = ctx;
+  std::string err;
+  slack_status st;
+  try {
+    st = build_plan(*pool_shape, n_streams, streams, o, ctx->sm_count, pl->hp, err);
+  } catch (const std::bad_alloc &) {
+    delete pl;
+    return set_err(ctx, SLACK_ENOMEM, "out of host memory while planning");
+  }
+  if (st != SLACK_OK) {
+    delete pl;
+    return set_err(ctx, st, err);
+  }
+  for (const DevStream &s : pl->hp.streams) pl->max_q_len = s.q_len > pl->max_q_len ? s.q_len : pl->max_q_len;
+
+  if (ctx->device >= 0) {
+    slack_status ds = ensure_device(ctx);
+    if (ds != SLACK_OK) {
+      delete pl;
+      return ds;
+    }
+    const HostPlan &hp = pl->hp;
+    const size_t b_streams = align_up(hp.streams.size() * sizeof(DevStream) + 16, 256);
+    const size_t b_pt = align_up(hp.page_tables.size() * sizeof(int32_t), 256);
+    const size_t b_items = align_up(hp.items.size() * sizeof(DevItem) + 16, 256);
+    const size_t b_cta = align_up(hp.cta_begin.size() * sizeof(int32_t), 256);
+    const size_t b_comb = align_up(hp.combines.size() * sizeof(DevCombine) + 16, 256);
+    const size_t total = b_streams + b_pt + b_items + b_cta + b_comb;
+    std::vector<uint8_t> blob(total, 0);
+    size_t off = 0;
+    auto put = [&](const void *src, size_t n, size_t padded) {
+      if (n) memcpy(blob.data() + off, src, n);
+      const size_t at = off;
+      off += padded;
+      return at;
+    };
+    const size_t o_streams = put(hp.streams.data(), hp.streams.size() * sizeof(DevStream), b_streams);
+    const size_t o_pt = put(hp.page_tables.data(), hp.page_tables.size() * sizeof(int32_t), b_pt);
+    const size_t o_items = put(hp.items.data(), hp.items.size() * sizeof(DevItem), b_items);
+    const size_t o_cta = put(hp.cta_begin.data(), hp.cta_begin.size() * sizeof(int32_t), b_cta);
+    const size_t o_comb = put(hp.combines.data(), hp.combines.size() * sizeof(DevCombine), b_comb);
+    cudaError_t e = cudaMalloc(&pl->d_blob, total);
+    if (e == cudaSuccess) e = cudaMemcpy(pl->d_blob, blob.data(), total, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+      if (pl->d_blob) cudaFree(pl->d_blob);
+      delete pl;
+      return cuda_err(ctx, e, "plan upload");
+    }
+    uint8_t *b = reinterpret_cast<uint8_t *>(pl->d_blob);
+    pl->d_streams = reinterpret_cast<DevStream *>(b + o_streams);
+    pl->d_page_tables = reinterpret_cast<int32_t *>(b + o_pt);
+    pl->d_items = reinterpret_cast<DevItem *>(b + o_items);
+    pl->d_cta_begin = reinterpret_cast<int32_t *>(b + o_cta);
+    pl->d_combines = reinterpret_cast<DevCombine *>(b + o_comb);
+  }
+  *plan_out = pl;
+  return SLACK_OK;
+}
+
+void slack_plan_destroy(slack_plan_t *plan) {
+  if (!plan) return;
+  if (plan->d_blob) {
+    if (plan->ctx && plan->ctx->device >= 0) cudaSetDevice(plan->ctx->device);
+    cudaFree(plan->d_blob); // synchronises with outstanding work that may still read the tables
+  }
+  delete plan;
+}
+
+size_t slack_plan_workspace_bytes(const slack_plan_t *plan) { return plan ? plan->hp.ws.total : 0; }
+int32_t slack_plan_num_items(const slack_plan_t *plan) { return plan ? (int32_t)plan->hp.items.size() : 0; }
+int32_t slack_plan_num_partial_slots(const slack_plan_t *plan) { return plan ? plan->hp.n_partial_slots : 0; }
+int32_t slack_plan_kernel_kind(const slack_plan_t *plan) { return plan ? plan->hp.kernel_kind : -1; }
+
+int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, int32_t capacity) {
+  if (!plan || !items || capacity <= 0) return 0;
+  const HostPlan &hp = plan->hp;
+  const int32_t n = (int32_t)hp.items.size() < capacity ? (int32_t)hp.items.size() : capacity;
+  for (int32_t i = 0; i < n; ++i) {
+    const DevItem &d = hp.items[i];
+    slack_work_item &w = items[i];
+    w.stream = d.stream;
+    w.head = d.head;
+    w.q_row0 = d.q_row0;
+    w.q_rows = d.q_rows;
+    w.kv_tile_begin = d.kv_tile_begin;
+    w.kv_tile_end = d.kv_tile_end;
+    w.pos_lo = d.pos_lo;
+    w.pos_hi = d.pos_hi;
+    w.partial_slot = d.partial_slot;
+    w.cta = hp.item_cta[i];
+  }
+  return n;
+}
+
+/* ------------------------------------------------------------------------------------------------ append */
+slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *k_new,
+                                     const void *v_new, void *cuda_stream) {
+  if (!ctx) return SLACK_EINVAL;
+  ctx->last_launches = 0;
+  if (!plan) return set_err(ctx, SLACK_EINVAL, "plan NULL");
+  slack_status st = ensure_device(ctx);
+  if (st != SLACK_OK) return st;
+  st = check_pool(ctx, pool, &plan->hp);
+  if (st != SLACK_OK) return st;
+  if (plan->hp.total_q == 0) return SLACK_OK;
+  if (!k_new || !v_new || !aligned(k_new, 16) || !aligned(v_new, 16))
+    return set_err(ctx, SLACK_EINVAL, "k_new / v_new NULL or not 16-byte aligned");
+  const HostPlan &hp = plan->hp;
+  SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, plan->d_streams, hp.n_streams, plan->max_q_len,
+                                   plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, elem_bytes(hp.dtype),
+                                   ctx->sm_count, reinterpret_cast<cudaStream_t>(cuda_stream), &ctx->last_launches));
+  return SLACK_OK;
+}
+
+slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_streams, const slack_stream *streams,
+                             const void *k_new, const void *v_new, void *cuda_stream) {
+  if (!ctx) return SLACK_EINVAL;
+  ctx->last_launches = 0;
+  slack_status st = ensure_device(ctx);
+  if (st != SLACK_OK) return st;
+  st = check_pool(ctx, pool, nullptr);
+  if (st != SLACK_OK) return st;
+  // validation and table building are the planner's (force_simt: no work items are needed for an append)
+  HostPlan hp;
+  std::string err;
+  slack_plan_opts o{};
+  o.force_simt = 1;
+  try {
+    st = build_plan(*pool, n_streams, streams, o, ctx->sm_count, hp, err);
+  } catch (const std::bad_alloc &) {
+    return set_err(ctx, SLACK_ENOMEM, "out of host memory");
+  }
+  if (st != SLACK_OK) return set_err(ctx, st, err);
+  if (hp.total_q == 0) return SLACK_OK;
+  if (!k_new || !v_new || !aligned(k_new, 16) || !aligned(v_new, 16))
+    return set_err(ctx, SLACK_EINVAL, "k_new / v_new NULL or not 16-byte aligned");
+  const size_t b_streams = align_up(hp.streams.size() * sizeof(DevStream), 256);
+  const size_t b_pt = align_up(hp.page_tables.size() * sizeof(int32_t), 256);
+  const size_t total = b_streams + b_pt;
+  cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (ctx->stage_pending) { // the previous append's copy must have consumed the staging buffer
+    SLACK_CUDA(ctx, cudaEventSynchronize(ctx->stage_ev));
+    ctx->stage_pending = false;
+  }
+  if (total > ctx->stage_cap) {
+    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->d_stage) cudaFree(ctx->d_stage); // device-synchronising: earlier appends have finished with it
+    ctx->h_stage = ctx->d_stage = nullptr;
+    ctx->stage_cap = 0;
+    const size_t cap = align_up(total * 2, 4096);
+    SLACK_CUDA(ctx, cudaMallocHost(&ctx->h_stage, cap));
+    SLACK_CUDA(ctx, cudaMalloc(&ctx->d_stage, cap));
+    ctx->stage_cap = cap;
+  }
+  uint8_t *h = reinterpret_cast<uint8_t *>(ctx->h_stage);
+  memcpy(h, hp.streams.data(), hp.streams.size() * sizeof(DevStream));
+  memcpy(h + b_streams, hp.page_tables.data(), hp.page_tables.size() * sizeof(int32_t));
+  SLACK_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage, h, total, cudaMemcpyHostToDevice, cs));
+  SLACK_CUDA(ctx, cudaEventRecord(ctx->stage_ev, cs));
+  ctx->stage_pending = true;
+  int max_q = 0;
+  for (const DevStream &s : hp.streams) max_q = s.q_len > max_q ? s.q_len : max_q;
+  uint8_t *d = reinterpret_cast<uint8_t *>(ctx->d_stage);
+  SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, reinterpret_cast<DevStream *>(d), hp.n_streams,
+                                   max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.head_dim, hp.page_size,
+                                   elem_bytes(hp.dtype), ctx->sm_count, cs, &ctx->last_launches));
+  return SLACK_OK;
+}
+
+/* ------------------------------------------------------------------------------------------------ attention */
+slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q, void *out,
+                                   float *lse, float scale, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SLACK_EINVAL;
+  ctx->last_launches = 0;
+  if (!plan) return set_err(ctx, SLACK_EINVAL, "plan NULL");
+  slack_status st = ensure_device(ctx);
+  if (st != SLACK_OK) return st;
+  st = check_pool(ctx, pool, &plan->hp);
+  if (st != SLACK_OK) return st;
+  const HostPlan &hp = plan->hp;
+  if (hp.total_q == 0) return SLACK_OK;
+  if (!q || !out || !aligned(q, 16) || !aligned(out, 16)) return set_err(ctx, SLACK_EINVAL, "q / out NULL or not 16-byte aligned");
+  if (!(scale > 0.f) || !(scale < 1e30f)) return set_err(ctx, SLACK_EINVAL, "scale must be a positive finite number");
+  cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
+
+  if (hp.kernel_kind == 1) {
+    SLACK_CUDA(ctx, launch_attn_simt(hp.dtype, q, pool->k_pool, pool->v_pool, out, lse, plan->d_streams, hp.n_streams, hp.total_q,
+                                     plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, scale, cs, &ctx->last_launches));
+    return SLACK_OK;
+  }
+
+  if (hp.ws.total > 0) {
+    if (!workspace || workspace_bytes < hp.ws.total) return set_err(ctx, SLACK_ENOMEM, "workspace NULL or smaller than slack_plan_workspace_bytes()");
+    if (!aligned(workspace, 16)) return set_err(ctx, SLACK_EINVAL, "workspace must be 16-byte aligned");
+  }
+  if (!aligned(q, 128) || !aligned(pool->k_pool, 128) || !aligned(pool->v_pool, 128))
+    return set_err(ctx, SLACK_EINVAL, "tensor-core path: q and pool pointers must be 128-byte aligned (TMA)");
+  if (!ctx->encode) return set_err(ctx, SLACK_ECUDA, "cuTensorMapEncodeTiled entry point not available");
+  if (!ctx->tc_configured) {
+    SLACK_CUDA(ctx, attn_tc_configure());
+    ctx->tc_configured = true;
+  }
+  CUtensorMap tm_q, tm_k, tm_v;
+  const uint64_t pool_rows = (uint64_t)hp.n_pages * hp.n_heads * hp.page_size;
+  if ((st = make_map(ctx, &tm_q, q, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  TcParams p{};
+  p.items = plan->d_items;
+  p.cta_begin = plan->d_cta_begin;
+  p.page_tables = plan->d_page_tables;
+  p.out = out;
+  p.lse = lse;
+  p.ws_o = reinterpret_cast<float *>(workspace);
+  p.ws_lse = workspace ? reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + hp.ws.lse_off) : nullptr;
+  p.dbg_s = ctx->dbg_s;
+  p.dbg_flag = ctx->d_dbg;
+  p.n_heads = hp.n_heads;
+  int pl2 = 0;
+  while ((1 << pl2) < hp.page_size) ++pl2;
+  p.page_log2 = pl2;
+  p.total_q = hp.total_q;
+  p.scale = scale;
+  SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
+  SLACK_CUDA(ctx, launch_combine(plan->d_combines, (int)hp.combines.size(), p.ws_o, p.ws_lse, out, lse, hp.n_heads, hp.head_dim,
+                                 hp.total_q, cs, &ctx->last_launches));
+  return SLACK_OK;
+}
+
+} // extern "C"

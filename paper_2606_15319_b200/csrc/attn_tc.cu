@@ -1,0 +1,439 @@
+// attn_tc.cu — A3: ragged chunk attention on the 5th-gen tensor cores (tcgen05 + TMEM + TMA), bf16, head_dim 128.
+//
+// What it computes (include/slack.h; PAPER.md P:21, P:84 chunk attends to cached earlier chunks; P:86 rolling window;
+// P:251 paged pool): for every planned item (stream, head, <=256 query rows, range of 128-key tiles)
+//     S = Q K^T (fp32 in TMEM)  ->  online softmax (one thread per query row)  ->  P (bf16, TMEM)  ->  O += P V (TMEM)
+// and, at the item's end, O / l written as bf16 (or as an fp32 partial + lse for split-KV items).
+//
+// CTA = 384 threads, persistent, one per SM, walking its planned queue:
+//   warp 0        TMA producer: Q tiles once per item, then K_j, V_j through a ring of 32 KB stages
+//   warp 1        MMA issuer (one lane issues tcgen05.mma); also owns TMEM alloc and zeroes masked V rows
+//   warps 2-3     idle (keep warpgroup 0 whole for setmaxnreg)
+//   warps 4-7     softmax + epilogue for query tile 0 (rows 0..127 of the item; thread = row = TMEM lane)
+//   warps 8-11    same for query tile 1 (rows 128..255)
+// The two query tiles ping-pong: while one tile's softmax runs on the ALU/MUFU pipes, the tensor pipe works on the
+// other tile's P V and next Q K^T.  TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_i is
+// written over the first 64 columns of S_i (two bf16 per 32-bit column).
+//
+// Shared memory layouts (all 128-byte swizzled, as TMA writes them and as the UMMA descriptors expect them):
+//   Q tile / K tile: two 16 KB halves (d 0..63, d 64..127), each [128 rows][128 B]  -> K-major operands
+//   V tile:          same bytes; read as the MN-major B operand of P V (N = d contiguous, K = keys)
+#include <cuda_bf16.h>
+
+#include "kernels.h"
+#include "ptx_sm100.cuh"
+
+namespace slack {
+using namespace ptx;
+
+namespace {
+
+constexpr int kStages = 5;
+constexpr uint32_t kTileBytes = 32768;
+constexpr uint32_t kHalfBytes = 16384;
+constexpr int kTcThreads = 384;
+
+constexpr uint32_t kOffQ = 0;
+constexpr uint32_t kOffKV = 2 * kTileBytes;
+constexpr uint32_t kOffBar = kOffKV + kStages * kTileBytes;
+
+enum : int {
+  BAR_Q_FULL = 0,
+  BAR_Q_EMPTY = 1,
+  BAR_KV_FULL = 2,
+  BAR_KV_EMPTY = BAR_KV_FULL + kStages,
+  BAR_S_FULL = BAR_KV_EMPTY + kStages, // [2]
+  BAR_P_READY = BAR_S_FULL + 2,        // [2]
+  BAR_O_FINAL = BAR_P_READY + 2,       // [2]
+  BAR_O_FREE = BAR_O_FINAL + 2,        // [2]
+  NUM_BARS = BAR_O_FREE + 2
+};
+constexpr uint32_t kOffTmemPtr = kOffBar + NUM_BARS * 8;
+constexpr uint32_t kSmemUsed = kOffTmemPtr + 16;
+constexpr uint32_t kSmemBytes = kSmemUsed + 1024; // slack for manual 1024-byte alignment
+
+constexpr uint32_t kIdescQK = make_idesc_bf16(128, 128, 0, 0);
+constexpr uint32_t kIdescPV = make_idesc_bf16(128, 128, 0, 1);
+
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kRescaleThreshold = 8.0f; // skip the O rescale while the row max grew by < 2^8 (in exp2 units)
+
+struct ItemView {
+  int tb, te, T, nq;
+};
+
+__device__ __forceinline__ ItemView view_of(const DevItem &it) {
+  ItemView v;
+  v.tb = it.kv_tile_begin;
+  v.te = it.kv_tile_end;
+  v.T = v.te - v.tb;
+  v.nq = it.q_rows > kTileM ? 2 : 1;
+  return v;
+}
+
+} // namespace
+
+__global__ void __launch_bounds__(kTcThreads, 1)
+attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+               const __grid_constant__ CUtensorMap tm_v) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = smem_base + kOffQ;
+  const uint32_t sKV = smem_base + kOffKV;
+  const uint32_t bars = smem_base + kOffBar;
+  const uint32_t tmem_ptr_smem = smem_base + kOffTmemPtr;
+  auto bar = [&](int i) { return bars + 8u * (uint32_t)i; };
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int item_begin = p.cta_begin[blockIdx.x];
+  const int item_end = p.cta_begin[blockIdx.x + 1];
+  unsigned long long *dbg = p.dbg_flag;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tensormap(&tm_q);
+    prefetch_tensormap(&tm_k);
+    prefetch_tensormap(&tm_v);
+    mbar_init(bar(BAR_Q_FULL), 1);
+    mbar_init(bar(BAR_Q_EMPTY), 1);
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(bar(BAR_KV_FULL + s), 1);
+      mbar_init(bar(BAR_KV_EMPTY + s), 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(bar(BAR_S_FULL + i), 1);
+      mbar_init(bar(BAR_P_READY + i), 4); // one arrival per softmax warp
+      mbar_init(bar(BAR_O_FINAL + i), 1);
+      mbar_init(bar(BAR_O_FREE + i), 4);
+    }
+    fence_barrier_init();
+  }
+  if (warp == 1) {
+    tmem_alloc(tmem_ptr_smem, 512);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+
+  const int H = p.n_heads;
+  const int P = 1 << p.page_log2;
+
+  if (warp < 4) {
+    setmaxnreg_dec<80>();
+    if (warp == 0) {
+      // ============================== TMA producer ==============================
+      uint32_t ring = 0;
+      int n_item = 0;
+      for (int k = item_begin; k < item_end; ++k, ++n_item) {
+        const DevItem it = p.items[k];
+        const ItemView v = view_of(it);
+        if (lane == 0) {
+          mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
+          mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes);
+          for (int i = 0; i < v.nq; ++i)
+            for (int c = 0; c < 2; ++c)
+              tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), it.head * 128 + c * 64,
+                          it.q_row0 + i * kTileM);
+        }
+        for (int t0 = v.tb; t0 < v.te; t0 += 32) {
+          const int my_t = t0 + lane;
+          int my_page = 0;
+          if (my_t < v.te) my_page = __ldg(p.page_tables + it.pt_off + ((my_t * kTileN) >> p.page_log2));
+          const int cnt = min(32, v.te - t0);
+          for (int j = 0; j < cnt; ++j) {
+            const int page = __shfl_sync(0xffffffffu, my_page, j);
+            if (lane == 0) {
+              const int row = (page * H + it.head) * P + (((t0 + j) * kTileN) & (P - 1));
+#pragma unroll
+              for (int kv = 0; kv < 2; ++kv) {
+                const uint32_t stage = ring % kStages;
+                const uint32_t ph = (ring / kStages) & 1u;
+                mbar_wait(bar(BAR_KV_EMPTY + stage), ph ^ 1u, 110 + stage, dbg);
+                mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes);
+                const CUtensorMap *tm = kv == 0 ? &tm_k : &tm_v;
+                tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
+                tma_load_2d(sKV + stage * kTileBytes + kHalfBytes, tm, bar(BAR_KV_FULL + stage), 64, row);
+                ++ring;
+              }
+            }
+          }
+        }
+      }
+    } else if (warp == 1) {
+      // ============================== MMA issuer ==============================
+      uint32_t ring = 0;
+      uint32_t cnt[2] = {0, 0}; // kv steps seen per query tile (parity of S_FULL / P_READY)
+      uint32_t itn[2] = {0, 0}; // items seen per query tile (parity of O_FINAL / O_FREE)
+      int n_item = 0;
+      auto issue_qk = [&](int i, uint32_t stage) {
+        const uint32_t a_base = sQ + i * kTileBytes;
+        const uint32_t b_base = sKV + stage * kTileBytes;
+        const uint32_t d = tmem_base + (uint32_t)(i * 128);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const uint32_t off = (uint32_t)(k >> 2) * kHalfBytes + (uint32_t)(k & 3) * 32u;
+          mma_ss(d, make_smem_desc_sw128(a_base + off, 16, 1024), make_smem_desc_sw128(b_base + off, 16, 1024), kIdescQK,
+                 k > 0 ? 1u : 0u);
+        }
+      };
+      auto issue_pv = [&](int i, uint32_t stage, bool acc) {
+        const uint32_t b_base = sKV + stage * kTileBytes;
+        const uint32_t d = tmem_base + (uint32_t)(256 + i * 128);
+        const uint32_t a = tmem_base + (uint32_t)(i * 128);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          mma_ts(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 2048u, kHalfBytes, 1024), kIdescPV,
+                 (acc || k > 0) ? 1u : 0u);
+        }
+      };
+      for (int k = item_begin; k < item_end; ++k, ++n_item) {
+        const DevItem it = p.items[k];
+        const ItemView v = view_of(it);
+        const uint32_t r0 = ring;
+        mbar_wait(bar(BAR_Q_FULL), (uint32_t)(n_item & 1), 200, dbg);
+        {
+          const uint32_t stage = r0 % kStages, ph = (r0 / kStages) & 1u;
+          mbar_wait(bar(BAR_KV_FULL + stage), ph, 210 + stage, dbg);
+          tc_fence_after();
+          if (lane == 0) {
+            for (int i = 0; i < v.nq; ++i) {
+              issue_qk(i, stage);
+              mma_commit(bar(BAR_S_FULL + i));
+            }
+            mma_commit(bar(BAR_KV_EMPTY + stage));
+            if (v.T == 1) mma_commit(bar(BAR_Q_EMPTY));
+          }
+          __syncwarp();
+        }
+        for (int j = 0; j < v.T; ++j) {
+          const uint32_t rv = r0 + 2u * (uint32_t)j + 1u;
+          const uint32_t stage_v = rv % kStages, ph_v = (rv / kStages) & 1u;
+          const bool has_next = (j + 1) < v.T;
+          const uint32_t rk = rv + 1u;
+          const uint32_t stage_k = rk % kStages, ph_k = (rk / kStages) & 1u;
+          mbar_wait(bar(BAR_KV_FULL + stage_v), ph_v, 220 + stage_v, dbg);
+          {
+            // masked key rows of V must be zero: P is 0 there, but 0 * NaN/Inf garbage would poison O
+            const int tile = v.tb + j;
+            const int c_lo = max(0, it.pos_lo - tile * kTileN);
+            const int c_hi = min(kTileN, it.pos_hi - tile * kTileN);
+            if (c_lo > 0 || c_hi < kTileN) {
+              const int n_zero = c_lo + (kTileN - c_hi);
+              const uint32_t base = sKV + stage_v * kTileBytes;
+              for (int idx = lane; idx < n_zero * 16; idx += 32) {
+                int r = idx >> 4;
+                r = r < c_lo ? r : c_hi + (r - c_lo);
+                const int w = idx & 15;
+                const uint32_t addr = base + (uint32_t)(w >> 3) * kHalfBytes + (uint32_t)r * 128u + (uint32_t)(w & 7) * 16u;
+                asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
+              }
+              fence_proxy_async_smem();
+              __syncwarp();
+            }
+          }
+          tc_fence_after();
+          for (int i = 0; i < v.nq; ++i) {
+            mbar_wait(bar(BAR_P_READY + i), cnt[i] & 1u, 230 + i, dbg);
+            if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
+            if (has_next && i == 0) mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
+            tc_fence_after();
+            if (lane == 0) {
+              issue_pv(i, stage_v, j > 0);
+              if (i == v.nq - 1) mma_commit(bar(BAR_KV_EMPTY + stage_v));
+              if (has_next) {
+                issue_qk(i, stage_k);
+                mma_commit(bar(BAR_S_FULL + i));
+                if (i == v.nq - 1) {
+                  mma_commit(bar(BAR_KV_EMPTY + stage_k));
+                  if (j + 2 == v.T) mma_commit(bar(BAR_Q_EMPTY));
+                }
+              } else {
+                mma_commit(bar(BAR_O_FINAL + i));
+              }
+            }
+            __syncwarp();
+            cnt[i]++;
+            if (!has_next) itn[i]++;
+          }
+        }
+        ring = r0 + 2u * (uint32_t)v.T;
+      }
+    }
+  } else {
+    // ============================== softmax + epilogue warpgroups ==============================
+    setmaxnreg_inc<208>();
+    const int i = warp >= 8 ? 1 : 0;
+    const int w4 = warp & 3;
+    const int row = w4 * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(w4 * 32) << 16;
+    const uint32_t tS = tmem_base + lane_addr + (uint32_t)(i * 128);
+    const uint32_t tO = tmem_base + lane_addr + (uint32_t)(256 + i * 128);
+    const float sl2 = p.scale * kLog2e;
+    uint32_t cnt = 0, itn = 0;
+    bool first_item = true;
+    for (int k = item_begin; k < item_end; ++k) {
+      const DevItem it = p.items[k];
+      const ItemView v = view_of(it);
+      if (i >= v.nq) continue;
+      float m = -INFINITY, l = 0.f;
+      for (int j = 0; j < v.T; ++j) {
+        mbar_wait(bar(BAR_S_FULL + i), cnt & 1u, 300 + i, dbg);
+        tc_fence_after();
+        float s[128];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t r[32];
+          tmem_ld32(tS + (uint32_t)(c * 32), r);
+#pragma unroll
+          for (int e = 0; e < 32; ++e) s[c * 32 + e] = __uint_as_float(r[e]);
+        }
+        tmem_wait_ld();
+        const int tile = v.tb + j;
+        const int c_lo = max(0, it.pos_lo - tile * kTileN);
+        const int c_hi = min(kTileN, it.pos_hi - tile * kTileN);
+        if (c_lo > 0 || c_hi < kTileN) {
+#pragma unroll
+          for (int e = 0; e < 128; ++e) s[e] = (e >= c_lo && e < c_hi) ? s[e] : -INFINITY;
+        }
+        if (p.dbg_s != nullptr && blockIdx.x == 0 && first_item && j == 0) {
+#pragma unroll
+          for (int e = 0; e < 128; ++e) p.dbg_s[(i * 128 + row) * 128 + e] = s[e];
+        }
+        float mx0 = max3(s[0], s[1], s[2]), mx1 = max3(s[3], s[4], s[5]);
+#pragma unroll
+        for (int e = 6; e + 3 < 128; e += 4) {
+          mx0 = max3(mx0, s[e], s[e + 1]);
+          mx1 = max3(mx1, s[e + 2], s[e + 3]);
+        }
+        const float mx = max3(mx0, mx1, fmaxf(s[126], s[127]));
+        if (j == 0) {
+          m = mx;
+        } else {
+          const bool need = (mx - m) * sl2 > kRescaleThreshold;
+          if (__any_sync(0xffffffffu, need)) {
+            // PV of the previous key tile has completed (its commit precedes S_FULL in the in-order tensor pipe)
+            const float alpha = need ? ex2((m - mx) * sl2) : 1.0f;
+            m = need ? mx : m;
+            l *= alpha;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              uint32_t r[32];
+              tmem_ld32(tO + (uint32_t)(c * 32), r);
+              tmem_wait_ld();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * alpha);
+              tmem_st32(tO + (uint32_t)(c * 32), r);
+            }
+          }
+        }
+        const float neg_m = -m * sl2;
+        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int e = 0; e < 32; e += 4) {
+            const float p0 = ex2(fmaf(s[c * 32 + e + 0], sl2, neg_m));
+            const float p1 = ex2(fmaf(s[c * 32 + e + 1], sl2, neg_m));
+            const float p2 = ex2(fmaf(s[c * 32 + e + 2], sl2, neg_m));
+            const float p3 = ex2(fmaf(s[c * 32 + e + 3], sl2, neg_m));
+            l0 += p0;
+            l1 += p1;
+            l2 += p2;
+            l3 += p3;
+            pk[(e >> 1) + 0] = pack_bf16x2(p0, p1);
+            pk[(e >> 1) + 1] = pack_bf16x2(p2, p3);
+          }
+          tmem_st16(tS + (uint32_t)(c * 16), pk);
+        }
+        l += (l0 + l1) + (l2 + l3);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(BAR_P_READY + i));
+        ++cnt;
+      }
+      // ---------------- epilogue: O / l ----------------
+      mbar_wait(bar(BAR_O_FINAL + i), itn & 1u, 310 + i, dbg);
+      tc_fence_after();
+      const float inv_l = 1.0f / l;
+      const int local_row = i * kTileM + row;
+      const bool valid = local_row < it.q_rows;
+      const float lse_val = (m * sl2 + log2f(l)) * kLn2;
+      if (it.partial_slot < 0) {
+        __nv_bfloat16 *dst =
+            reinterpret_cast<__nv_bfloat16 *>(p.out) + ((size_t)(it.q_row0 + local_row) * H + it.head) * 128;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t r[32];
+          tmem_ld32(tO + (uint32_t)(c * 32), r);
+          tmem_wait_ld();
+          if (valid) {
+#pragma unroll
+            for (int e = 0; e < 32; e += 8) {
+              uint4 o;
+              o.x = pack_bf16x2(__uint_as_float(r[e + 0]) * inv_l, __uint_as_float(r[e + 1]) * inv_l);
+              o.y = pack_bf16x2(__uint_as_float(r[e + 2]) * inv_l, __uint_as_float(r[e + 3]) * inv_l);
+              o.z = pack_bf16x2(__uint_as_float(r[e + 4]) * inv_l, __uint_as_float(r[e + 5]) * inv_l);
+              o.w = pack_bf16x2(__uint_as_float(r[e + 6]) * inv_l, __uint_as_float(r[e + 7]) * inv_l);
+              *reinterpret_cast<uint4 *>(dst + c * 32 + e) = o;
+            }
+          }
+        }
+        if (valid && p.lse != nullptr) p.lse[(size_t)it.head * p.total_q + it.q_row0 + local_row] = lse_val;
+      } else {
+        float *dst = p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * 128;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t r[32];
+          tmem_ld32(tO + (uint32_t)(c * 32), r);
+          tmem_wait_ld();
+          if (valid) {
+#pragma unroll
+            for (int e = 0; e < 32; e += 4) {
+              float4 o;
+              o.x = __uint_as_float(r[e + 0]) * inv_l;
+              o.y = __uint_as_float(r[e + 1]) * inv_l;
+              o.z = __uint_as_float(r[e + 2]) * inv_l;
+              o.w = __uint_as_float(r[e + 3]) * inv_l;
+              *reinterpret_cast<float4 *>(dst + c * 32 + e) = o;
+            }
+          }
+        }
+        if (valid) p.ws_lse[(size_t)it.partial_slot * kItemRows + local_row] = lse_val;
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(BAR_O_FREE + i));
+      ++itn;
+      first_item = false;
+    }
+  }
+
+  // ---------------- teardown ----------------
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+size_t attn_tc_smem_bytes() { return kSmemBytes; }
+
+cudaError_t attn_tc_configure() {
+  return cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+}
+
+cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
+                           int n_cta, cudaStream_t st, int *n_launched) {
+  attn_tc_kernel<<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+  if (n_launched) *n_launched += 1;
+  return cudaGetLastError();
+}
+
+} // namespace slack

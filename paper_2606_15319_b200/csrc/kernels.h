@@ -1,0 +1,45 @@
+// kernels.h — launch functions of the CUDA kernels (defined in append.cu, attn_simt.cu, attn_tc.cu, combine.cu).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "slack_internal.h"
+
+namespace slack {
+
+// A1: paged scatter copy. elem_bytes = 2 (bf16) or 4 (f32). Launches 1 kernel (0 if nothing to copy).
+cudaError_t launch_kv_append(const void *k_new, const void *v_new, void *k_pool, void *v_pool, const DevStream *d_streams,
+                             int n_streams, int max_q_len, const int32_t *d_page_tables, int n_heads, int head_dim,
+                             int page_size, int elem_bytes, int sm_count, cudaStream_t st, int *n_launched);
+
+// A3 (validation / fp32 path): one warp per (query row, head), fp32 accumulation, any page size.
+cudaError_t launch_attn_simt(int dtype, const void *q, const void *k_pool, const void *v_pool, void *out, float *lse,
+                             const DevStream *d_streams, int n_streams, int total_q, const int32_t *d_page_tables,
+                             int n_heads, int head_dim, int page_size, float scale, cudaStream_t st, int *n_launched);
+
+// A3 (tensor-core path, bf16, head_dim 128, page_size >= 128).
+struct TcParams {
+  const DevItem *items;
+  const int32_t *cta_begin;
+  const int32_t *page_tables;
+  void *out;            // bf16 [total_q][H][128]
+  float *lse;           // [H][total_q] or null
+  float *ws_o;          // partial outputs [slot][256][128] fp32
+  float *ws_lse;        // partial lse [slot][256]
+  float *dbg_s;         // optional debug dump of the first S tiles of CTA 0 ([2][128][128] fp32), else null
+  unsigned long long *dbg_flag; // optional 4-word device buffer for time-out diagnostics, else null
+  int32_t n_heads;
+  int32_t page_log2;
+  int32_t total_q;
+  float scale;          // logits = scale * q.k
+};
+size_t attn_tc_smem_bytes();
+cudaError_t attn_tc_configure(); // cudaFuncSetAttribute(max dynamic smem); once per process/device
+cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
+                           int n_cta, cudaStream_t st, int *n_launched);
+
+// A4: merge split-KV partials into `out` (bf16) and `lse`.
+cudaError_t launch_combine(const DevCombine *d_combines, int n_combines, const float *ws_o, const float *ws_lse, void *out,
+                           float *lse, int n_heads, int head_dim, int total_q, cudaStream_t st, int *n_launched);
+
+} // namespace slack

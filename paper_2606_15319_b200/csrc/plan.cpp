@@ -1,0 +1,265 @@
+// plan.cpp — A2: host-side ragged batch planner (integer work only; no CUDA).
+//
+// Not in the paper: the paper's Execution Plane dispatches one stream at a time per worker (§3.2,
+// P:638 App. C.1); co-batching streams of different cache lengths in one launch is BASELINE.json north_star's
+// extension.  The planner turns the batch into work items (stream, head, 256-row query block, range of 128-key
+// tiles), decides where key ranges are cut (split-KV), and list-schedules the items onto one queue per SM.
+//
+// Item order = locality order: streams by descending key-tile count, then head, then key chunk, then query block.
+// Consecutive items therefore share the same (stream, head, key chunk); with equal-cost items the greedy earliest-
+// free assignment degenerates to round-robin, so co-running CTAs sweep the same K/V tiles at the same time and each
+// tile is fetched from HBM once and then hit in L2.
+#include <algorithm>
+#include <cstdio>
+#include <functional>
+#include <numeric>
+#include <queue>
+
+#include "slack_internal.h"
+
+namespace slack {
+namespace {
+
+struct StreamGeom {
+  int32_t idx;
+  int32_t tile0, tiles;   // position-tile range
+  int32_t q_blocks;       // ceil(q_len / 256)
+};
+
+constexpr double kTileCost = 2.0;      // one 128-key tile against a 256-row item (two MMA tile pairs)
+constexpr double kItemOverhead = 5.0;  // pipeline fill/drain + epilogue, in the same unit
+constexpr double kPartialCost = 3.0;   // extra epilogue traffic + combine work per partial slot
+
+struct Candidate {
+  std::vector<DevItem> items;
+  std::vector<int32_t> item_cta;
+  std::vector<DevCombine> combines;
+  int32_t n_slots = 0;
+  double makespan = 0, ideal = 0, objective = 0;
+};
+
+int32_t ceil_div(int64_t a, int64_t b) { return (int32_t)((a + b - 1) / b); }
+
+// parts[s] = number of key chunks for stream s
+void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int32_t> &parts,
+                    const std::vector<DevStream> &ds, int32_t n_heads, int32_t n_cta, Candidate &c) {
+  c = Candidate();
+  for (size_t oi = 0; oi < order.size(); ++oi) {
+    const StreamGeom &g = order[oi];
+    const DevStream &s = ds[g.idx];
+    const int32_t np = parts[oi];
+    for (int32_t h = 0; h < n_heads; ++h) {
+      int32_t slot0 = -1;
+      if (np > 1) {
+        slot0 = c.n_slots;
+        c.n_slots += np * g.q_blocks;
+        for (int32_t qb = 0; qb < g.q_blocks; ++qb) {
+          DevCombine cb{};
+          cb.q_row0 = s.q_row0 + qb * kItemRows;
+          cb.q_rows = std::min(kItemRows, s.q_len - qb * kItemRows);
+          cb.head = h;
+          cb.slot_begin = slot0 + qb * np;
+          cb.n_parts = np;
+          c.combines.push_back(cb);
+        }
+      }
+      for (int32_t p = 0; p < np; ++p) {
+        const int32_t tb = g.tile0 + (int32_t)(((int64_t)p * g.tiles) / np);
+        const int32_t te = g.tile0 + (int32_t)(((int64_t)(p + 1) * g.tiles) / np);
+        for (int32_t qb = 0; qb < g.q_blocks; ++qb) {
+          DevItem it{};
+          it.q_row0 = s.q_row0 + qb * kItemRows;
+          it.q_rows = std::min(kItemRows, s.q_len - qb * kItemRows);
+          it.head = h;
+          it.pt_off = s.pt_off;
+          it.kv_tile_begin = tb;
+          it.kv_tile_end = te;
+          it.pos_lo = s.pos_lo;
+          it.pos_hi = s.pos_hi;
+          it.partial_slot = (np > 1) ? slot0 + qb * np + p : -1;
+          it.stream = g.idx;
+          c.items.push_back(it);
+        }
+      }
+    }
+  }
+  // greedy list scheduling in item order: each item goes to the queue that frees up first
+  using Slot = std::pair<double, int32_t>;
+  std::priority_queue<Slot, std::vector<Slot>, std::greater<Slot>> heap;
+  for (int32_t i = 0; i < n_cta; ++i) heap.push({0.0, i});
+  c.item_cta.resize(c.items.size());
+  double total = 0;
+  for (size_t i = 0; i < c.items.size(); ++i) {
+    const double cost = kTileCost * (c.items[i].kv_tile_end - c.items[i].kv_tile_begin) + kItemOverhead;
+    Slot s = heap.top();
+    heap.pop();
+    c.item_cta[i] = s.second;
+    s.first += cost;
+    total += cost;
+    c.makespan = std::max(c.makespan, s.first);
+    heap.push(s);
+  }
+  c.ideal = total / n_cta;
+  c.objective = c.makespan + kPartialCost * c.n_slots / n_cta;
+}
+
+bool is_pow2(int32_t x) { return x > 0 && (x & (x - 1)) == 0; }
+
+} // namespace
+
+slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_stream *streams,
+                        const slack_plan_opts &opts, int32_t default_sm_count, HostPlan &out, std::string &err) {
+  char buf[256];
+  auto fail = [&](slack_status st, const char *msg) {
+    err = msg;
+    return st;
+  };
+  if (n_streams < 0 || (n_streams > 0 && !streams)) return fail(SLACK_EINVAL, "n_streams < 0 or streams == NULL");
+  if (shape.n_pages <= 0 || shape.n_heads <= 0) return fail(SLACK_EINVAL, "pool: n_pages and n_heads must be > 0");
+  if (shape.dtype != SLACK_BF16 && shape.dtype != SLACK_F32) return fail(SLACK_EINVAL, "pool: unknown dtype");
+  if (shape.head_dim != 64 && shape.head_dim != 128) return fail(SLACK_EUNSUPPORTED, "head_dim must be 64 or 128");
+  if (!is_pow2(shape.page_size) || shape.page_size < 16)
+    return fail(SLACK_EUNSUPPORTED, "page_size must be a power of two >= 16");
+  if (opts.sm_count < 0 || opts.force_splits < 0) return fail(SLACK_EINVAL, "plan opts: negative sm_count/force_splits");
+
+  out = HostPlan();
+  out.n_pages = shape.n_pages;
+  out.n_heads = shape.n_heads;
+  out.head_dim = shape.head_dim;
+  out.page_size = shape.page_size;
+  out.dtype = shape.dtype;
+  out.n_streams = n_streams;
+  out.n_cta = opts.sm_count > 0 ? opts.sm_count : default_sm_count;
+  const bool tc_ok = shape.dtype == SLACK_BF16 && shape.head_dim == 128 && shape.page_size >= kTileN;
+  out.kernel_kind = (tc_ok && !opts.force_simt) ? 0 : 1;
+
+  // ---- validate streams, build device stream records and the concatenated page table ------------------------
+  std::vector<uint8_t> owned((size_t)shape.n_pages, 0);
+  int64_t row = 0;
+  const int32_t P = shape.page_size;
+  for (int32_t i = 0; i < n_streams; ++i) {
+    const slack_stream &s = streams[i];
+    if (s.q_len < 0 || s.cache_len < 0 || s.window < 0 || s.n_table_pages < 0) {
+      snprintf(buf, sizeof buf, "stream %d: negative q_len/cache_len/window/n_table_pages", i);
+      return fail(SLACK_EINVAL, buf);
+    }
+    if (s.base < 0 || s.base >= P) {
+      snprintf(buf, sizeof buf, "stream %d: base %d outside [0, page_size)", i, s.base);
+      return fail(SLACK_EINVAL, buf);
+    }
+    if (s.sink_len != 0) {
+      snprintf(buf, sizeof buf, "stream %d: sink_len != 0 is reserved", i);
+      return fail(SLACK_EUNSUPPORTED, buf);
+    }
+    const int64_t n = (int64_t)s.cache_len + s.q_len;
+    if ((int64_t)s.base + n > (int64_t)INT32_MAX / 2 || row + s.q_len > (int64_t)INT32_MAX / 2)
+      return fail(SLACK_EINVAL, "batch too large for 32-bit token positions");
+    const int32_t need = n > 0 ? ceil_div((int64_t)s.base + n, P) : 0;
+    if (s.n_table_pages < need) {
+      snprintf(buf, sizeof buf, "stream %d: page table has %d pages, needs %d", i, s.n_table_pages, need);
+      return fail(SLACK_EINVAL, buf);
+    }
+    if (need > 0 && !s.page_table) {
+      snprintf(buf, sizeof buf, "stream %d: page_table == NULL", i);
+      return fail(SLACK_EINVAL, buf);
+    }
+    DevStream d{};
+    d.q_row0 = (int32_t)row;
+    d.q_len = s.q_len;
+    d.cache_len = s.cache_len;
+    d.base = s.base;
+    const int64_t lo = (s.window > 0) ? std::max<int64_t>(0, n - s.window) : 0;
+    d.pos_lo = (int32_t)(s.base + lo);
+    d.pos_hi = (int32_t)(s.base + n);
+    d.pt_off = (int32_t)out.page_tables.size();
+    d.n_table_pages = need;
+    for (int32_t p = 0; p < need; ++p) {
+      const int32_t id = s.page_table[p];
+      if (id < 0 || id >= shape.n_pages) {
+        snprintf(buf, sizeof buf, "stream %d: page_table[%d] = %d outside [0, %d)", i, p, id, shape.n_pages);
+        return fail(SLACK_EINVAL, buf);
+      }
+      if (owned[id]) {
+        snprintf(buf, sizeof buf, "stream %d: physical page %d is owned twice in the batch", i, id);
+        return fail(SLACK_EINVAL, buf);
+      }
+      owned[id] = 1;
+      out.page_tables.push_back(id);
+    }
+    out.streams.push_back(d);
+    row += s.q_len;
+  }
+  out.total_q = (int32_t)row;
+  if (out.page_tables.empty()) out.page_tables.push_back(0); // keep device arrays non-empty
+
+  out.cta_begin.assign((size_t)out.n_cta + 1, 0);
+  if (out.kernel_kind == 1) return SLACK_OK; // the SIMT kernel walks DevStream records directly: no items
+
+  // ---- tensor-core path: geometry per stream ------------------------------------------------------------------
+  std::vector<StreamGeom> order;
+  for (int32_t i = 0; i < n_streams; ++i) {
+    const DevStream &d = out.streams[i];
+    if (d.q_len == 0) continue;
+    StreamGeom g;
+    g.idx = i;
+    g.tile0 = d.pos_lo / kTileN;
+    g.tiles = ceil_div(d.pos_hi, kTileN) - g.tile0;
+    g.q_blocks = ceil_div(d.q_len, kItemRows);
+    order.push_back(g);
+  }
+  std::stable_sort(order.begin(), order.end(), [](const StreamGeom &a, const StreamGeom &b) { return a.tiles > b.tiles; });
+  if (order.empty()) return SLACK_OK;
+
+  const int32_t t_max = order.front().tiles;
+  Candidate best;
+  bool have = false;
+  std::vector<int32_t> parts(order.size());
+  auto consider = [&](int32_t k, bool exact) {
+    for (size_t i = 0; i < order.size(); ++i) {
+      if (exact) {
+        parts[i] = std::min(k, order[i].tiles);
+      } else {
+        const int32_t target = ceil_div(t_max, k); // chunk length the longest stream gets
+        parts[i] = std::max(1, std::min(order[i].tiles, (int32_t)((order[i].tiles + target / 2) / target)));
+      }
+    }
+    Candidate c;
+    make_candidate(order, parts, out.streams, shape.n_heads, out.n_cta, c);
+    if (!have || c.objective < best.objective - 1e-9) {
+      best = std::move(c);
+      have = true;
+    }
+  };
+  if (opts.force_splits > 0) {
+    consider(opts.force_splits, true);
+  } else {
+    const int32_t ks[] = {1, 2, 3, 4, 5, 6, 8, 10, 12, 16};
+    for (int32_t k : ks)
+      if (k <= t_max) consider(k, false);
+  }
+
+  // ---- emit per-CTA queues (stable: queue order = item order) ------------------------------------------------
+  const size_t n_items = best.items.size();
+  std::vector<int32_t> count((size_t)out.n_cta, 0);
+  for (size_t i = 0; i < n_items; ++i) count[best.item_cta[i]]++;
+  for (int32_t c = 0; c < out.n_cta; ++c) out.cta_begin[c + 1] = out.cta_begin[c] + count[c];
+  std::vector<int32_t> cursor(out.cta_begin.begin(), out.cta_begin.end() - 1);
+  out.items.resize(n_items);
+  out.item_cta.resize(n_items);
+  for (size_t i = 0; i < n_items; ++i) {
+    const int32_t c = best.item_cta[i];
+    out.items[cursor[c]] = best.items[i];
+    out.item_cta[cursor[c]] = c;
+    cursor[c]++;
+  }
+  out.combines = std::move(best.combines);
+  out.n_partial_slots = best.n_slots;
+  out.makespan = best.makespan;
+  out.ideal = best.ideal;
+  out.ws.o_bytes = (size_t)out.n_partial_slots * kItemRows * shape.head_dim * sizeof(float);
+  out.ws.lse_off = out.ws.o_bytes;
+  out.ws.total = out.ws.o_bytes + (size_t)out.n_partial_slots * kItemRows * sizeof(float);
+  return SLACK_OK;
+}
+
+} // namespace slack

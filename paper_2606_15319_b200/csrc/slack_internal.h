@@ -1,0 +1,87 @@
+// slack_internal.h — structures shared by the host planner (plan.cpp), the entry points (api.cu) and the kernels.
+// Nothing here is part of the ABI (include/slack.h is).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/slack.h"
+
+namespace slack {
+
+// Geometry of the tensor-core path (fixed at compile time).
+constexpr int kTileM = 128;    // query rows per MMA tile (UMMA M)
+constexpr int kTileN = 128;    // keys per KV tile (UMMA N of QK^T, K extent of PV); anchored to page slots
+constexpr int kItemRows = 256; // an item carries two query tiles that ping-pong on the tensor pipe
+
+// One planned unit of work as the kernels read it (device copy of slack_work_item plus table offsets). 48 bytes.
+struct DevItem {
+  int32_t q_row0;        // global row (ragged concat) of the item's first query row
+  int32_t q_rows;        // valid rows, 1..256
+  int32_t head;
+  int32_t pt_off;        // offset of the stream's page table inside the concatenated device table
+  int32_t kv_tile_begin; // position-tile range [begin, end), tile T = positions [128T, 128T+128)
+  int32_t kv_tile_end;
+  int32_t pos_lo;        // visible positions [pos_lo, pos_hi)
+  int32_t pos_hi;
+  int32_t partial_slot;  // -1 = final output, else workspace slot
+  int32_t stream;
+  int32_t pad0, pad1;
+};
+static_assert(sizeof(DevItem) == 48, "DevItem layout");
+
+// One output row-block whose key range was cut: the combine kernel merges its partial slots (A4).
+struct DevCombine {
+  int32_t q_row0;     // global first row
+  int32_t q_rows;     // valid rows (<= 256)
+  int32_t head;
+  int32_t slot_begin; // partial slots [slot_begin, slot_begin + n_parts)
+  int32_t n_parts;
+  int32_t pad[3];
+};
+static_assert(sizeof(DevCombine) == 32, "DevCombine layout");
+
+// Per-stream record used by the append kernel and the SIMT kernel.
+struct DevStream {
+  int32_t q_row0;   // first row of the stream in the ragged concat
+  int32_t q_len;
+  int32_t cache_len;
+  int32_t base;
+  int32_t pos_lo;   // base + lo
+  int32_t pos_hi;   // base + n
+  int32_t pt_off;
+  int32_t n_table_pages;
+};
+static_assert(sizeof(DevStream) == 32, "DevStream layout");
+
+// Workspace layout for split-KV partials: slot s holds kItemRows rows of head_dim fp32 (normalised partial output)
+// followed, in a second region, by kItemRows fp32 lse values.
+struct WorkspaceLayout {
+  size_t o_bytes = 0;   // n_slots * 256 * D * 4
+  size_t lse_off = 0;   // = o_bytes
+  size_t total = 0;
+};
+
+struct HostPlan {
+  // shape the plan was made for
+  int32_t n_pages = 0, n_heads = 0, head_dim = 0, page_size = 0, dtype = 0;
+  int32_t n_streams = 0, total_q = 0;
+  int32_t n_cta = 0;
+  int32_t kernel_kind = 0; // 0 tensor-core, 1 SIMT
+  std::vector<DevStream> streams;
+  std::vector<int32_t> page_tables;  // concatenated
+  std::vector<DevItem> items;        // in queue order: CTA c owns items [cta_begin[c], cta_begin[c+1])
+  std::vector<int32_t> cta_begin;    // n_cta + 1
+  std::vector<int32_t> item_cta;     // per item
+  std::vector<DevCombine> combines;
+  int32_t n_partial_slots = 0;
+  WorkspaceLayout ws;
+  double makespan = 0, ideal = 0;    // in cost units (for tests / tuning)
+};
+
+// Validates and plans. Returns SLACK_OK or an error with `err` filled in.
+slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_stream *streams,
+                        const slack_plan_opts &opts, int32_t default_sm_count, HostPlan &out, std::string &err);
+
+} // namespace slack
