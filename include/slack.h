@@ -150,6 +150,14 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
 /* Number of kernels the last slack_chunk_attention / slack_kv_append call on this ctx launched (bench bookkeeping). */
 int32_t slack_last_launch_count(const slack_ctx *ctx);
 
+/* ---- measurement (bench.py's roofline figure) ------------------------------------------------------- */
+/* enable != 0: every following slack_chunk_attention records a CUDA event pair on the caller's stream directly
+ * around the tensor-core attention kernel (not the combine kernel).  slack_profile_read waits for the recorded pairs,
+ * returns the summed kernel time in milliseconds and the number of launches timed, and resets the record.  Off by
+ * default: the events cost two stream operations per call. */
+slack_status slack_profile_attention(slack_ctx *ctx, int32_t enable);
+slack_status slack_profile_read(slack_ctx *ctx, double *total_ms, int32_t *n_launches);
+
 /* ---- diagnostics (never on the data path) ---------------------------------------------------------------------- */
 /* key 0: `value` = DEVICE pointer to a [2][128][128] fp32 buffer that receives the first two S = QK^T tiles computed by
  * CTA 0 of the next tensor-core launches (NULL switches the dump off). */

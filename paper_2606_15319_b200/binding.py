@@ -64,6 +64,8 @@ SYMBOLS = {
     "slack_plan_kernel_kind": (C.c_int32, [_VP]),
     "slack_plan_get_items": (C.c_int32, [_VP, C.POINTER(CWorkItem), C.c_int32]),
     "slack_chunk_attention": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP, C.c_size_t, _VP]),
+    "slack_profile_attention": (C.c_int, [_VP, C.c_int32]),
+    "slack_profile_read": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_int32)]),
     "slack_debug_set": (C.c_int, [_VP, C.c_int32, _VP]),
     "slack_debug_timeout": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
 }
@@ -224,6 +226,16 @@ class Context:
         ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
         self._check(self.lib.slack_chunk_attention(self.handle, plan.handle, C.byref(pool.c), _ptr(q), _ptr(out), _ptr(lse),
                                                    C.c_float(scale), _ptr(workspace), ws_bytes, _cuda_stream(stream)))
+
+    # --- measurement ---------------------------------------------------------------------------------------------------
+    def profile_attention(self, enable: bool) -> None:
+        self._check(self.lib.slack_profile_attention(self.handle, int(bool(enable))))
+
+    def profile_read(self):
+        """(total milliseconds, launches) of the attention kernel since the last read."""
+        ms, n = C.c_double(0), C.c_int32(0)
+        self._check(self.lib.slack_profile_read(self.handle, C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
 
     # --- diagnostics --------------------------------------------------------------------------------------------------
     def debug_set_s_dump(self, tensor) -> None:

@@ -7,6 +7,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "kernels.h"
 #include "slack_internal.h"
@@ -34,6 +35,10 @@ struct slack_ctx {
   unsigned long long *h_dbg = nullptr; // mapped pinned, 4 words, survives a trapped launch
   unsigned long long *d_dbg = nullptr;
   float *dbg_s = nullptr;
+  // per-launch timing of the attention kernel (slack_profile_attention)
+  bool prof_on = false;
+  std::vector<cudaEvent_t> prof_events; // pairs: [2i] before, [2i+1] after
+  size_t prof_used = 0;                 // pairs recorded since the last read
 };
 
 struct slack_plan_s {
@@ -153,6 +158,7 @@ void slack_destroy(slack_ctx *ctx) {
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->d_stage) cudaFree(ctx->d_stage);
     if (ctx->h_dbg) cudaFreeHost(ctx->h_dbg);
+    for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
   }
   delete ctx;
 }
@@ -173,6 +179,29 @@ slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value) {
 slack_status slack_debug_timeout(slack_ctx *ctx, uint64_t out[4]) {
   if (!ctx || !out) return SLACK_EINVAL;
   for (int i = 0; i < 4; ++i) out[i] = ctx->h_dbg ? ctx->h_dbg[i] : 0;
+  return SLACK_OK;
+}
+
+slack_status slack_profile_attention(slack_ctx *ctx, int32_t enable) {
+  if (!ctx) return SLACK_EINVAL;
+  ctx->prof_on = enable != 0;
+  return SLACK_OK;
+}
+slack_status slack_profile_read(slack_ctx *ctx, double *total_ms, int32_t *n_launches) {
+  if (!ctx || !total_ms || !n_launches) return SLACK_EINVAL;
+  *total_ms = 0;
+  *n_launches = 0;
+  if (ctx->prof_used == 0) return SLACK_OK;
+  slack_status st = ensure_device(ctx);
+  if (st != SLACK_OK) return st;
+  for (size_t i = 0; i < ctx->prof_used; ++i) {
+    float ms = 0.f;
+    SLACK_CUDA(ctx, cudaEventSynchronize(ctx->prof_events[2 * i + 1]));
+    SLACK_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->prof_events[2 * i], ctx->prof_events[2 * i + 1]));
+    *total_ms += ms;
+  }
+  *n_launches = (int32_t)ctx->prof_used;
+  ctx->prof_used = 0;
   return SLACK_OK;
 }
 
@@ -409,7 +438,21 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
   p.page_log2 = pl2;
   p.total_q = hp.total_q;
   p.scale = scale;
+  cudaEvent_t ev_after = nullptr;
+  if (ctx->prof_on) {
+    while (ctx->prof_events.size() < 2 * (ctx->prof_used + 1)) {
+      cudaEvent_t e;
+      SLACK_CUDA(ctx, cudaEventCreate(&e));
+      ctx->prof_events.push_back(e);
+    }
+    SLACK_CUDA(ctx, cudaEventRecord(ctx->prof_events[2 * ctx->prof_used], cs));
+    ev_after = ctx->prof_events[2 * ctx->prof_used + 1];
+  }
   SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
+  if (ev_after) {
+    SLACK_CUDA(ctx, cudaEventRecord(ev_after, cs));
+    ctx->prof_used++;
+  }
   SLACK_CUDA(ctx, launch_combine(plan->d_combines, (int)hp.combines.size(), p.ws_o, p.ws_lse, out, lse, hp.n_heads, hp.head_dim,
                                  hp.total_q, cs, &ctx->last_launches));
   return SLACK_OK;
