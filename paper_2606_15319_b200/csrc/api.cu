@@ -31,6 +31,8 @@ struct slack_ctx {
   size_t stage_cap = 0;
   cudaEvent_t stage_ev = nullptr;
   bool stage_pending = false;
+  // plan tables are uploaded on a private non-blocking stream: slack_plan never waits for the caller's queued work
+  cudaStream_t up_stream = nullptr;
   // diagnostics
   unsigned long long *h_dbg = nullptr; // mapped pinned, 4 words, survives a trapped launch
   unsigned long long *d_dbg = nullptr;
@@ -133,6 +135,7 @@ slack_status slack_create(slack_ctx **out, int device) {
       if (e == cudaSuccess && qres == cudaDriverEntryPointSuccess) ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->stage_ev, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->up_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) {
       e = cudaHostAlloc(reinterpret_cast<void **>(&ctx->h_dbg), 4 * sizeof(unsigned long long), cudaHostAllocMapped);
       if (e == cudaSuccess) {
@@ -155,6 +158,7 @@ void slack_destroy(slack_ctx *ctx) {
     cudaSetDevice(ctx->device);
     if (ctx->stage_pending) cudaEventSynchronize(ctx->stage_ev);
     if (ctx->stage_ev) cudaEventDestroy(ctx->stage_ev);
+    if (ctx->up_stream) cudaStreamDestroy(ctx->up_stream);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->d_stage) cudaFree(ctx->d_stage);
     if (ctx->h_dbg) cudaFreeHost(ctx->h_dbg);
@@ -257,7 +261,8 @@ slack_status slack_plan(slack_ctx *ctx, const slack_pool *pool_shape, int32_t n_
     const size_t o_cta = put(hp.cta_begin.data(), hp.cta_begin.size() * sizeof(int32_t), b_cta);
     const size_t o_comb = put(hp.combines.data(), hp.combines.size() * sizeof(DevCombine), b_comb);
     cudaError_t e = cudaMalloc(&pl->d_blob, total);
-    if (e == cudaSuccess) e = cudaMemcpy(pl->d_blob, blob.data(), total, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_blob, blob.data(), total, cudaMemcpyHostToDevice, ctx->up_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->up_stream); // the tables are resident when slack_plan returns
     if (e != cudaSuccess) {
       if (pl->d_blob) cudaFree(pl->d_blob);
       delete pl;

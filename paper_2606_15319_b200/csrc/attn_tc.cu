@@ -85,7 +85,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
   const uint32_t tmem_ptr_smem = smem_base + kOffTmemPtr;
   auto bar = [&](int i) { return bars + 8u * (uint32_t)i; };
 
-  const int warp = threadIdx.x >> 5;
+  // warp-uniform by construction, and provably so for the compiler (keeps the role branches and everything the
+  // MMA issuer derives from them on the uniform datapath: UTCHMMA takes its descriptors from uniform registers)
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   const int lane = threadIdx.x & 31;
   const int item_begin = p.cta_begin[blockIdx.x];
   const int item_end = p.cta_begin[blockIdx.x + 1];
@@ -126,39 +128,46 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
     setmaxnreg_dec<80>();
     if (warp == 0) {
       // ============================== TMA producer ==============================
+      // The whole warp walks the loop (uniform control flow); one elected lane arms the barrier and issues the copies.
       uint32_t ring = 0;
       int n_item = 0;
       for (int k = item_begin; k < item_end; ++k, ++n_item) {
         const DevItem it = p.items[k];
-        const ItemView v = view_of(it);
-        if (lane == 0) {
-          mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
+        ItemView v = view_of(it);
+        v.tb = uni(v.tb);
+        v.te = uni(v.te);
+        v.nq = uni(v.nq);
+        const int head = uni(it.head), q_row0 = uni(it.q_row0), pt_off = uni(it.pt_off);
+        mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
+        if (elect_one()) {
           mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes);
           for (int i = 0; i < v.nq; ++i)
             for (int c = 0; c < 2; ++c)
-              tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), it.head * 128 + c * 64,
-                          it.q_row0 + i * kTileM);
+              tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), head * 128 + c * 64,
+                          q_row0 + i * kTileM);
         }
+        __syncwarp();
         for (int t0 = v.tb; t0 < v.te; t0 += 32) {
           const int my_t = t0 + lane;
           int my_page = 0;
-          if (my_t < v.te) my_page = __ldg(p.page_tables + it.pt_off + ((my_t * kTileN) >> p.page_log2));
+          if (my_t < v.te) my_page = __ldg(p.page_tables + pt_off + ((my_t * kTileN) >> p.page_log2));
           const int cnt = min(32, v.te - t0);
           for (int j = 0; j < cnt; ++j) {
             const int page = __shfl_sync(0xffffffffu, my_page, j);
-            if (lane == 0) {
-              const int row = (page * H + it.head) * P + (((t0 + j) * kTileN) & (P - 1));
+            const int row = (page * H + head) * P + (((t0 + j) * kTileN) & (P - 1));
 #pragma unroll
-              for (int kv = 0; kv < 2; ++kv) {
-                const uint32_t stage = ring % kStages;
-                const uint32_t ph = (ring / kStages) & 1u;
-                mbar_wait(bar(BAR_KV_EMPTY + stage), ph ^ 1u, 110 + stage, dbg);
+            for (int kv = 0; kv < 2; ++kv) {
+              const uint32_t stage = ring % kStages;
+              const uint32_t ph = (ring / kStages) & 1u;
+              mbar_wait(bar(BAR_KV_EMPTY + stage), ph ^ 1u, 110 + stage, dbg);
+              if (elect_one()) {
                 mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes);
                 const CUtensorMap *tm = kv == 0 ? &tm_k : &tm_v;
                 tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
                 tma_load_2d(sKV + stage * kTileBytes + kHalfBytes, tm, bar(BAR_KV_FULL + stage), 64, row);
-                ++ring;
               }
+              __syncwarp();
+              ++ring;
             }
           }
         }
@@ -192,14 +201,18 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       };
       for (int k = item_begin; k < item_end; ++k, ++n_item) {
         const DevItem it = p.items[k];
-        const ItemView v = view_of(it);
+        ItemView v = view_of(it);
+        v.tb = uni(v.tb);
+        v.T = uni(v.T);
+        v.nq = uni(v.nq);
+        const int pos_lo = uni(it.pos_lo), pos_hi = uni(it.pos_hi);
         const uint32_t r0 = ring;
         mbar_wait(bar(BAR_Q_FULL), (uint32_t)(n_item & 1), 200, dbg);
         {
           const uint32_t stage = r0 % kStages, ph = (r0 / kStages) & 1u;
           mbar_wait(bar(BAR_KV_FULL + stage), ph, 210 + stage, dbg);
           tc_fence_after();
-          if (lane == 0) {
+          if (elect_one()) {
             for (int i = 0; i < v.nq; ++i) {
               issue_qk(i, stage);
               mma_commit(bar(BAR_S_FULL + i));
@@ -219,8 +232,8 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           {
             // masked key rows of V must be zero: P is 0 there, but 0 * NaN/Inf garbage would poison O
             const int tile = v.tb + j;
-            const int c_lo = max(0, it.pos_lo - tile * kTileN);
-            const int c_hi = min(kTileN, it.pos_hi - tile * kTileN);
+            const int c_lo = max(0, pos_lo - tile * kTileN);
+            const int c_hi = min(kTileN, pos_hi - tile * kTileN);
             if (c_lo > 0 || c_hi < kTileN) {
               const int n_zero = c_lo + (kTileN - c_hi);
               const uint32_t base = sKV + stage_v * kTileBytes;
@@ -241,7 +254,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
             if (has_next && i == 0) mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
             tc_fence_after();
-            if (lane == 0) {
+            if (elect_one()) {
               issue_pv(i, stage_v, j > 0);
               if (i == v.nq - 1) mma_commit(bar(BAR_KV_EMPTY + stage_v));
               if (has_next) {
