@@ -241,6 +241,10 @@ class Context:
     def debug_set_s_dump(self, tensor) -> None:
         self._check(self.lib.slack_debug_set(self.handle, 0, _ptr(tensor)))
 
+    def debug_set_trace(self, tensor) -> None:
+        """int32/uint32 device tensor [3, 64, 8] (or None): clock trace of CTA 0's first item, see include/slack.h."""
+        self._check(self.lib.slack_debug_set(self.handle, 1, _ptr(tensor)))
+
     def debug_timeout(self):
         buf = (C.c_uint64 * 4)()
         self.lib.slack_debug_timeout(self.handle, buf)

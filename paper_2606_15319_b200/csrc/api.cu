@@ -37,6 +37,7 @@ struct slack_ctx {
   unsigned long long *h_dbg = nullptr; // mapped pinned, 4 words, survives a trapped launch
   unsigned long long *d_dbg = nullptr;
   float *dbg_s = nullptr;
+  uint32_t *dbg_t = nullptr;
   // per-launch timing of the attention kernel (slack_profile_attention)
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_events; // pairs: [2i] before, [2i+1] after
@@ -171,11 +172,15 @@ const char *slack_last_error(const slack_ctx *ctx) { return ctx ? ctx->err.c_str
 int32_t slack_last_launch_count(const slack_ctx *ctx) { return ctx ? ctx->last_launches : 0; }
 
 /* diagnostics (not part of the data path): key 0 = device pointer of a [2][128][128] fp32 buffer receiving the first
- * S tiles of CTA 0 (NULL disables); slack_debug_timeout copies the 4-word time-out record of the last trapped launch. */
+ * S tiles of CTA 0 (NULL disables); key 1 = device pointer of a [3][64][8] uint32 clock trace of CTA 0's first item; slack_debug_timeout copies the 4-word time-out record of the last trapped launch. */
 slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value) {
   if (!ctx) return SLACK_EINVAL;
   if (key == 0) {
     ctx->dbg_s = reinterpret_cast<float *>(value);
+    return SLACK_OK;
+  }
+  if (key == 1) {
+    ctx->dbg_t = reinterpret_cast<uint32_t *>(value);
     return SLACK_OK;
   }
   return set_err(ctx, SLACK_EINVAL, "unknown debug key");
@@ -436,6 +441,7 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
   p.ws_o = reinterpret_cast<float *>(workspace);
   p.ws_lse = workspace ? reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + hp.ws.lse_off) : nullptr;
   p.dbg_s = ctx->dbg_s;
+  p.dbg_t = ctx->dbg_t;
   p.dbg_flag = ctx->d_dbg;
   p.n_heads = hp.n_heads;
   int pl2 = 0;

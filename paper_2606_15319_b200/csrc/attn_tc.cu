@@ -57,6 +57,10 @@ constexpr uint32_t kIdescPV = make_idesc_bf16(128, 128, 0, 1);
 
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
+#ifndef SLACK_EMU_OF_8
+#define SLACK_EMU_OF_8 2
+#endif
+constexpr int kEmuOf8 = SLACK_EMU_OF_8; // pairs out of every 8 whose exp2 runs on the FMA pipe instead of the MUFU
 constexpr float kRescaleThreshold = 8.0f; // skip the O rescale while the row max grew by < 2^8 (in exp2 units)
 
 struct ItemView {
@@ -74,6 +78,15 @@ __device__ __forceinline__ ItemView view_of(const DevItem &it) {
 
 } // namespace
 
+// kTrace: diagnostic build that records clock64() time stamps of CTA 0's first item into p.dbg_t (slack_debug_set key 1):
+// [role 0/1 = softmax tile 0/1, 2 = MMA issuer][kv step < 64][8 slots].  The production instantiation has no trace code.
+#define SLACK_TRACE(role, step, slot)                                                                      \
+  if constexpr (kTrace) {                                                                                  \
+    if (blockIdx.x == 0 && k == item_begin && (step) < 64 && (threadIdx.x & ((role) == 2 ? 31 : 127)) == 0)                    \
+      p.dbg_t[((role) * 64 + (step)) * 8 + (slot)] = (uint32_t)clock64();                                  \
+  }
+
+template <bool kTrace>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                const __grid_constant__ CUtensorMap tm_v) {
@@ -228,7 +241,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           const bool has_next = (j + 1) < v.T;
           const uint32_t rk = rv + 1u;
           const uint32_t stage_k = rk % kStages, ph_k = (rk / kStages) & 1u;
+          SLACK_TRACE(2, j, 0);
           mbar_wait(bar(BAR_KV_FULL + stage_v), ph_v, 220 + stage_v, dbg);
+          SLACK_TRACE(2, j, 1);
           {
             // masked key rows of V must be zero: P is 0 there, but 0 * NaN/Inf garbage would poison O
             const int tile = v.tb + j;
@@ -254,6 +269,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
             if (has_next && i == 0) mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
             tc_fence_after();
+            SLACK_TRACE(2, j, 2 + 2 * i);
             if (elect_one()) {
               issue_pv(i, stage_v, j > 0);
               if (i == v.nq - 1) mma_commit(bar(BAR_KV_EMPTY + stage_v));
@@ -269,6 +285,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
               }
             }
             __syncwarp();
+            SLACK_TRACE(2, j, 3 + 2 * i);
             cnt[i]++;
             if (!has_next) itn[i]++;
           }
@@ -294,8 +311,10 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       if (i >= v.nq) continue;
       float m = -INFINITY, l = 0.f;
       for (int j = 0; j < v.T; ++j) {
+        SLACK_TRACE(i, j, 0);
         mbar_wait(bar(BAR_S_FULL + i), cnt & 1u, 300 + i, dbg);
         tc_fence_after();
+        SLACK_TRACE(i, j, 1);
         float s[128];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
@@ -305,6 +324,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           for (int e = 0; e < 32; ++e) s[c * 32 + e] = __uint_as_float(r[e]);
         }
         tmem_wait_ld();
+        SLACK_TRACE(i, j, 2);
         const int tile = v.tb + j;
         const int c_lo = max(0, it.pos_lo - tile * kTileN);
         const int c_hi = min(kTileN, it.pos_hi - tile * kTileN);
@@ -316,13 +336,19 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 #pragma unroll
           for (int e = 0; e < 128; ++e) p.dbg_s[(i * 128 + row) * 128 + e] = s[e];
         }
-        float mx0 = max3(s[0], s[1], s[2]), mx1 = max3(s[3], s[4], s[5]);
+        // row max of the tile: four independent FMNMX3 chains
+        float mxc[4];
 #pragma unroll
-        for (int e = 6; e + 3 < 128; e += 4) {
-          mx0 = max3(mx0, s[e], s[e + 1]);
-          mx1 = max3(mx1, s[e + 2], s[e + 3]);
+        for (int c = 0; c < 4; ++c) mxc[c] = max3(s[c * 32], s[c * 32 + 1], s[c * 32 + 2]);
+#pragma unroll
+        for (int e = 3; e + 1 < 32; e += 2) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) mxc[c] = max3(mxc[c], s[c * 32 + e], s[c * 32 + e + 1]);
         }
-        const float mx = max3(mx0, mx1, fmaxf(s[126], s[127]));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) mxc[c] = fmaxf(mxc[c], s[c * 32 + 31]);
+        const float mx = fmaxf(max3(mxc[0], mxc[1], mxc[2]), mxc[3]);
+        SLACK_TRACE(i, j, 3);
         if (j == 0) {
           m = mx;
         } else {
@@ -343,31 +369,47 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             }
           }
         }
+        SLACK_TRACE(i, j, 4);
         const float neg_m = -m * sl2;
-        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+        // P = 2^(s*sl2 - m*sl2) on packed pairs: FFMA2 for the argument, then either 2 MUFU.EX2 or (kEmuOf8 pairs out
+        // of every 8) the FMA-pipe polynomial; FADD2 row sums; one F2FP per pair.
+        const uint64_t sl2_2 = pack2(sl2, sl2), negm_2 = pack2(neg_m, neg_m);
+        uint64_t la0 = pack2(0.f, 0.f), la1 = la0;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t pk[16];
 #pragma unroll
-          for (int e = 0; e < 32; e += 4) {
-            const float p0 = ex2(fmaf(s[c * 32 + e + 0], sl2, neg_m));
-            const float p1 = ex2(fmaf(s[c * 32 + e + 1], sl2, neg_m));
-            const float p2 = ex2(fmaf(s[c * 32 + e + 2], sl2, neg_m));
-            const float p3 = ex2(fmaf(s[c * 32 + e + 3], sl2, neg_m));
-            l0 += p0;
-            l1 += p1;
-            l2 += p2;
-            l3 += p3;
-            pk[(e >> 1) + 0] = pack_bf16x2(p0, p1);
-            pk[(e >> 1) + 1] = pack_bf16x2(p2, p3);
+          for (int e = 0; e < 16; ++e) {
+            const uint64_t x2 = ffma2(pack2(s[c * 32 + 2 * e], s[c * 32 + 2 * e + 1]), sl2_2, negm_2);
+            uint64_t p2;
+            if ((e & 7) < kEmuOf8) {
+              p2 = exp2_poly2(x2);
+            } else {
+              float x0, x1;
+              unpack2(x2, x0, x1);
+              p2 = pack2(ex2(x0), ex2(x1));
+            }
+            if (e & 1) la1 = fadd2(la1, p2); else la0 = fadd2(la0, p2);
+            float p0, p1;
+            unpack2(p2, p0, p1);
+            pk[e] = pack_bf16x2(p0, p1);
           }
           tmem_st16(tS + (uint32_t)(c * 16), pk);
         }
-        l += (l0 + l1) + (l2 + l3);
+        {
+          float a0, a1;
+          unpack2(fadd2(la0, la1), a0, a1);
+          l += a0 + a1;
+        }
+        SLACK_TRACE(i, j, 5);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(BAR_P_READY + i));
+        SLACK_TRACE(i, j, 6);
+        if constexpr (kTrace) { // per-warp arrival times (rows 3.. : [3][j][warp - 4])
+          if (blockIdx.x == 0 && k == item_begin && j < 64 && lane == 0) p.dbg_t[(3 * 64 + j) * 8 + (warp - 4)] = (uint32_t)clock64();
+        }
         ++cnt;
       }
       // ---------------- epilogue: O / l ----------------
@@ -439,12 +481,17 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 size_t attn_tc_smem_bytes() { return kSmemBytes; }
 
 cudaError_t attn_tc_configure() {
-  return cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
 }
 
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched) {
-  attn_tc_kernel<<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+  if (p.dbg_t != nullptr)
+    attn_tc_kernel<true><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+  else
+    attn_tc_kernel<false><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
   if (n_launched) *n_launched += 1;
   return cudaGetLastError();
 }

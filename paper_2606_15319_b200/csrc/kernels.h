@@ -27,6 +27,7 @@ struct TcParams {
   float *ws_o;          // partial outputs [slot][256][128] fp32
   float *ws_lse;        // partial lse [slot][256]
   float *dbg_s;         // optional debug dump of the first S tiles of CTA 0 ([2][128][128] fp32), else null
+  uint32_t *dbg_t;      // optional time-stamp trace [3][64][8] (selects the kTrace instantiation), else null
   unsigned long long *dbg_flag; // optional 4-word device buffer for time-out diagnostics, else null
   int32_t n_heads;
   int32_t page_log2;

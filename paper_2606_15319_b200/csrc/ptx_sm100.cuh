@@ -177,6 +177,53 @@ __device__ __forceinline__ float max3(float a, float b, float c) {
   asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
   return d;
 }
+// ---------------------------------------------------------------- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2)
+// One issue slot per two lanes of work; operands are even-aligned register pairs.
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float &lo, float &hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+// 2^x for a pair, x <= ~8, evaluated on the FMA/ALU pipes instead of the MUFU: round x to the nearest integer n with
+// the 1.5*2^23 trick, degree-3 minimax polynomial of 2^f on f = x - n in [-0.5, 0.5] (max relative error 7.5e-5, far
+// below the bf16 rounding of P), then n is added into the exponent field.  x is clamped at -125 (result ~2^-125).
+__device__ __forceinline__ uint64_t exp2_poly2(uint64_t x2) {
+  float x0, x1;
+  unpack2(x2, x0, x1);
+  x0 = fmaxf(x0, -125.0f);
+  x1 = fmaxf(x1, -125.0f);
+  x2 = pack2(x0, x1);
+  const uint64_t magic = pack2(12582912.0f, 12582912.0f), nmagic = pack2(-12582912.0f, -12582912.0f);
+  const uint64_t mone = pack2(-1.0f, -1.0f);
+  const uint64_t c0 = pack2(0.9999281764030457f, 0.9999281764030457f), c1 = pack2(0.6932609677314758f, 0.6932609677314758f);
+  const uint64_t c2 = pack2(0.24260930716991425f, 0.24260930716991425f), c3 = pack2(0.055170927196741104f, 0.055170927196741104f);
+  const uint64_t t2 = fadd2(x2, magic);
+  const uint64_t n2 = fadd2(t2, nmagic);
+  const uint64_t f2 = ffma2(n2, mone, x2);
+  uint64_t p2 = ffma2(c3, f2, c2);
+  p2 = ffma2(p2, f2, c1);
+  p2 = ffma2(p2, f2, c0);
+  float p0, p1, t0, t1;
+  unpack2(p2, p0, p1);
+  unpack2(t2, t0, t1);
+  const uint32_t r0 = (__float_as_uint(t0) << 23) + __float_as_uint(p0);
+  const uint32_t r1 = (__float_as_uint(t1) << 23) + __float_as_uint(p1);
+  return pack2(__uint_as_float(r0), __uint_as_float(r1));
+}
+
 // pack two fp32 -> bf16x2, `lo` in bits [0,16), `hi` in bits [16,32) (round to nearest even)
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t d;
