@@ -43,8 +43,9 @@ enum : int {
   BAR_KV_FULL = 2,
   BAR_KV_EMPTY = BAR_KV_FULL + kStages,
   BAR_S_FULL = BAR_KV_EMPTY + kStages, // [2]
-  BAR_P_READY = BAR_S_FULL + 2,        // [2]
-  BAR_O_FINAL = BAR_P_READY + 2,       // [2]
+  BAR_P_READY = BAR_S_FULL + 2,        // [2] all of P written (keys 64..127 were the last)
+  BAR_P_LO = BAR_P_READY + 2,          // [2] P of keys 0..63 written: the first half of P V may start
+  BAR_O_FINAL = BAR_P_LO + 2,          // [2]
   BAR_O_FREE = BAR_O_FINAL + 2,        // [2]
   NUM_BARS = BAR_O_FREE + 2
 };
@@ -119,6 +120,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar(BAR_S_FULL + i), 1);
       mbar_init(bar(BAR_P_READY + i), 4); // one arrival per softmax warp
+      mbar_init(bar(BAR_P_LO + i), 4);
       mbar_init(bar(BAR_O_FINAL + i), 1);
       mbar_init(bar(BAR_O_FREE + i), 4);
     }
@@ -202,12 +204,14 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                  k > 0 ? 1u : 0u);
         }
       };
-      auto issue_pv = [&](int i, uint32_t stage, bool acc) {
+      // P V over keys [64*half, 64*half + 64) of the tile (4 MMAs of K = 16)
+      auto issue_pv = [&](int i, uint32_t stage, int half, bool acc) {
         const uint32_t b_base = sKV + stage * kTileBytes;
         const uint32_t d = tmem_base + (uint32_t)(256 + i * 128);
         const uint32_t a = tmem_base + (uint32_t)(i * 128);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
+        for (int kk = 0; kk < 4; ++kk) {
+          const int k = half * 4 + kk;
           mma_ts(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 2048u, kHalfBytes, 1024), kIdescPV,
                  (acc || k > 0) ? 1u : 0u);
         }
@@ -265,13 +269,17 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           }
           tc_fence_after();
           for (int i = 0; i < v.nq; ++i) {
-            mbar_wait(bar(BAR_P_READY + i), cnt[i] & 1u, 230 + i, dbg);
+            mbar_wait(bar(BAR_P_LO + i), cnt[i] & 1u, 260 + i, dbg);
             if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
-            if (has_next && i == 0) mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
             tc_fence_after();
             SLACK_TRACE(2, j, 2 + 2 * i);
+            if (elect_one()) issue_pv(i, stage_v, 0, j > 0);
+            __syncwarp();
+            mbar_wait(bar(BAR_P_READY + i), cnt[i] & 1u, 230 + i, dbg);
+            if (has_next && i == 0) mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
+            tc_fence_after();
             if (elect_one()) {
-              issue_pv(i, stage_v, j > 0);
+              issue_pv(i, stage_v, 1, true);
               if (i == v.nq - 1) mma_commit(bar(BAR_KV_EMPTY + stage_v));
               if (has_next) {
                 issue_qk(i, stage_k);
@@ -336,47 +344,30 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 #pragma unroll
           for (int e = 0; e < 128; ++e) p.dbg_s[(i * 128 + row) * 128 + e] = s[e];
         }
-        // row max of the tile: four independent FMNMX3 chains
-        float mxc[4];
+        // Row max of the tile: four independent FMNMX3 chains.  On the first tile of an item it is needed before any
+        // exponential; later it is evaluated in the same instruction stream as the first 64 columns' exponentials
+        // (which use the running max), and only a growth beyond the threshold forces those 64 columns to be redone.
+        auto row_max = [&]() {
+          float mxc[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) mxc[c] = max3(s[c * 32], s[c * 32 + 1], s[c * 32 + 2]);
+          for (int c = 0; c < 4; ++c) mxc[c] = max3(s[c * 32], s[c * 32 + 1], s[c * 32 + 2]);
 #pragma unroll
-        for (int e = 3; e + 1 < 32; e += 2) {
+          for (int e = 3; e + 1 < 32; e += 2) {
 #pragma unroll
-          for (int c = 0; c < 4; ++c) mxc[c] = max3(mxc[c], s[c * 32 + e], s[c * 32 + e + 1]);
-        }
-#pragma unroll
-        for (int c = 0; c < 4; ++c) mxc[c] = fmaxf(mxc[c], s[c * 32 + 31]);
-        const float mx = fmaxf(max3(mxc[0], mxc[1], mxc[2]), mxc[3]);
-        SLACK_TRACE(i, j, 3);
-        if (j == 0) {
-          m = mx;
-        } else {
-          const bool need = (mx - m) * sl2 > kRescaleThreshold;
-          if (__any_sync(0xffffffffu, need)) {
-            // PV of the previous key tile has completed (its commit precedes S_FULL in the in-order tensor pipe)
-            const float alpha = need ? ex2((m - mx) * sl2) : 1.0f;
-            m = need ? mx : m;
-            l *= alpha;
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              uint32_t r[32];
-              tmem_ld32(tO + (uint32_t)(c * 32), r);
-              tmem_wait_ld();
-#pragma unroll
-              for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * alpha);
-              tmem_st32(tO + (uint32_t)(c * 32), r);
-            }
+            for (int c = 0; c < 4; ++c) mxc[c] = max3(mxc[c], s[c * 32 + e], s[c * 32 + e + 1]);
           }
-        }
-        SLACK_TRACE(i, j, 4);
-        const float neg_m = -m * sl2;
+#pragma unroll
+          for (int c = 0; c < 4; ++c) mxc[c] = fmaxf(mxc[c], s[c * 32 + 31]);
+          return fmaxf(max3(mxc[0], mxc[1], mxc[2]), mxc[3]);
+        };
+        if (j == 0) m = row_max();
+        SLACK_TRACE(i, j, 3);
         // P = 2^(s*sl2 - m*sl2) on packed pairs: FFMA2 for the argument, then either 2 MUFU.EX2 or (kEmuOf8 pairs out
         // of every 8) the FMA-pipe polynomial; FADD2 row sums; one F2FP per pair.
-        const uint64_t sl2_2 = pack2(sl2, sl2), negm_2 = pack2(neg_m, neg_m);
+        const uint64_t sl2_2 = pack2(sl2, sl2);
+        uint64_t negm_2 = pack2(-m * sl2, -m * sl2);
         uint64_t la0 = pack2(0.f, 0.f), la1 = la0;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        auto exp_chunk = [&](int c) { // 32 columns -> 16 packed bf16x2 columns of P
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 16; ++e) {
@@ -395,7 +386,39 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             pk[e] = pack_bf16x2(p0, p1);
           }
           tmem_st16(tS + (uint32_t)(c * 16), pk);
+        };
+        {
+          const float mx = row_max(); // independent of the two chunks below: the scheduler interleaves them
+          exp_chunk(0);
+          exp_chunk(1);
+          const bool need = (mx - m) * sl2 > kRescaleThreshold; // never on the first tile (m == mx)
+          if (__any_sync(0xffffffffu, need)) {
+            // PV of the previous key tile has completed (its commit precedes S_FULL in the in-order tensor pipe)
+            const float alpha = need ? ex2((m - mx) * sl2) : 1.0f;
+            m = need ? mx : m;
+            l *= alpha;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              uint32_t r[32];
+              tmem_ld32(tO + (uint32_t)(c * 32), r);
+              tmem_wait_ld();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * alpha);
+              tmem_st32(tO + (uint32_t)(c * 32), r);
+            }
+            negm_2 = pack2(-m * sl2, -m * sl2);
+            la0 = la1 = pack2(0.f, 0.f);
+            exp_chunk(0);
+            exp_chunk(1);
+          }
         }
+        SLACK_TRACE(i, j, 4);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(BAR_P_LO + i)); // P V over keys 0..63 may start
+        exp_chunk(2);
+        exp_chunk(3);
         {
           float a0, a1;
           unpack2(fadd2(la0, la1), a0, a1);

@@ -4,7 +4,8 @@
 //     m = max_p lse_p ;  out = sum_p e^{lse_p - m} O_p / sum_p e^{lse_p - m} ;  lse = m + ln sum_p e^{lse_p - m}.
 // (Not in the paper: BASELINE.json north_star "split-KV with a combine pass for long caches"; the formula is pinned
 // against the unsplit definition in tests/test_oracle_pins.py.)  HBM-bound: (4*D + 4)*parts bytes read and 2*D written
-// per row.  One CTA per (row block, head); a warp owns a row at a time, its 32 lanes split head_dim as float4.
+// per row.  Grid = (combine entries, 256 / kRowsPerCta); a warp owns one row, its 32 lanes split head_dim as float4, and
+// the loads of all parts of a row are independent (the partials were just written and mostly still sit in L2).
 #include <cuda_bf16.h>
 
 #include "kernels.h"
@@ -13,37 +14,62 @@ namespace slack {
 namespace {
 
 constexpr int kCombineThreads = 256;
+constexpr int kRowsPerCta = kCombineThreads / 32; // one row per warp
+constexpr int kMaxPartsUnrolled = 4;
 
 template <int D>
 __global__ void __launch_bounds__(kCombineThreads)
 combine_kernel(const DevCombine *__restrict__ combines, const float *__restrict__ ws_o, const float *__restrict__ ws_lse,
                __nv_bfloat16 *__restrict__ out, float *__restrict__ lse, int n_heads, int total_q) {
-  constexpr int E = D / 32;
+  static_assert(D == 128, "one float4 per lane");
   const DevCombine cb = combines[blockIdx.x];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int r = warp; r < cb.q_rows; r += kCombineThreads / 32) {
-    float m = -INFINITY;
-    for (int p = 0; p < cb.n_parts; ++p) m = fmaxf(m, ws_lse[(size_t)(cb.slot_begin + p) * kItemRows + r]);
-    float den = 0.f, acc[E];
+  const int r = blockIdx.y * kRowsPerCta + warp;
+  if (r >= cb.q_rows) return;
+  const float *lse_p = ws_lse + (size_t)cb.slot_begin * kItemRows + r;
+  const float4 *o_p = reinterpret_cast<const float4 *>(ws_o + ((size_t)cb.slot_begin * kItemRows + r) * D) + lane;
+  constexpr size_t kSlotStride4 = (size_t)kItemRows * D / 4;
+  float m = -INFINITY;
+  for (int p = 0; p < cb.n_parts; ++p) m = fmaxf(m, __ldg(lse_p + (size_t)p * kItemRows));
+  float den = 0.f;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  int p = 0;
+  for (; p + kMaxPartsUnrolled <= cb.n_parts; p += kMaxPartsUnrolled) { // batches of independent loads
+    float4 v[kMaxPartsUnrolled];
+    float w[kMaxPartsUnrolled];
 #pragma unroll
-    for (int e = 0; e < E; ++e) acc[e] = 0.f;
-    for (int p = 0; p < cb.n_parts; ++p) {
-      const size_t slot = (size_t)(cb.slot_begin + p);
-      const float w = expf(ws_lse[slot * kItemRows + r] - m);
-      den += w;
-      const float *src = ws_o + (slot * kItemRows + r) * D + lane * E;
-#pragma unroll
-      for (int e = 0; e < E; ++e) acc[e] = fmaf(w, src[e], acc[e]);
+    for (int u = 0; u < kMaxPartsUnrolled; ++u) {
+      v[u] = __ldg(o_p + (size_t)(p + u) * kSlotStride4);
+      w[u] = __ldg(lse_p + (size_t)(p + u) * kItemRows);
     }
-    const float inv = 1.0f / den;
-    __nv_bfloat16 *dst = out + ((size_t)(cb.q_row0 + r) * n_heads + cb.head) * D + lane * E;
 #pragma unroll
-    for (int e = 0; e < E; e += 2) {
-      __nv_bfloat162 v = __floats2bfloat162_rn(acc[e] * inv, acc[e + 1] * inv);
-      *reinterpret_cast<__nv_bfloat162 *>(dst + e) = v;
+    for (int u = 0; u < kMaxPartsUnrolled; ++u) {
+      const float e = expf(w[u] - m);
+      den += e;
+      acc.x = fmaf(e, v[u].x, acc.x);
+      acc.y = fmaf(e, v[u].y, acc.y);
+      acc.z = fmaf(e, v[u].z, acc.z);
+      acc.w = fmaf(e, v[u].w, acc.w);
     }
-    if (lse != nullptr && lane == 0) lse[(size_t)cb.head * total_q + cb.q_row0 + r] = m + logf(den);
   }
+  for (; p < cb.n_parts; ++p) {
+    const float4 v = __ldg(o_p + (size_t)p * kSlotStride4);
+    const float e = expf(__ldg(lse_p + (size_t)p * kItemRows) - m);
+    den += e;
+    acc.x = fmaf(e, v.x, acc.x);
+    acc.y = fmaf(e, v.y, acc.y);
+    acc.z = fmaf(e, v.z, acc.z);
+    acc.w = fmaf(e, v.w, acc.w);
+  }
+  const float inv = 1.0f / den;
+  __nv_bfloat16 *dst = out + ((size_t)(cb.q_row0 + r) * n_heads + cb.head) * D + lane * 4;
+  const __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv);
+  const __nv_bfloat162 hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
+  uint2 o;
+  o.x = *reinterpret_cast<const uint32_t *>(&lo);
+  o.y = *reinterpret_cast<const uint32_t *>(&hi);
+  *reinterpret_cast<uint2 *>(dst) = o;
+  if (lse != nullptr && lane == 0) lse[(size_t)cb.head * total_q + cb.q_row0 + r] = m + logf(den);
 }
 
 } // namespace
@@ -52,7 +78,7 @@ cudaError_t launch_combine(const DevCombine *d_combines, int n_combines, const f
                            float *lse, int n_heads, int head_dim, int total_q, cudaStream_t st, int *n_launched) {
   if (n_combines == 0) return cudaSuccess;
   if (head_dim != 128) return cudaErrorInvalidValue;
-  combine_kernel<128><<<n_combines, kCombineThreads, 0, st>>>(d_combines, ws_o, ws_lse,
+  combine_kernel<128><<<dim3((unsigned)n_combines, kItemRows / kRowsPerCta), kCombineThreads, 0, st>>>(d_combines, ws_o, ws_lse,
                                                               reinterpret_cast<__nv_bfloat16 *>(out), lse, n_heads, total_q);
   if (n_launched) *n_launched += 1;
   return cudaGetLastError();

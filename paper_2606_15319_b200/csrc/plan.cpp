@@ -5,11 +5,11 @@
 // extension.  The planner turns the batch into work items (stream, head, 256-row query block, range of 128-key
 // tiles), decides where key ranges are cut (split-KV), and list-schedules the items onto one queue per SM.
 //
-// Item order = locality order: streams by descending key-tile count, then head, then key chunk, then query block.
-// Consecutive items therefore share the same (stream, head, key chunk); with equal-cost items the greedy earliest-
-// free assignment degenerates to round-robin, so co-running CTAs sweep the same K/V tiles at the same time and each
-// tile is fetched from HBM once and then hit in L2.
+// Item order = locality order: streams by descending key-tile count, then head, then query block (then key chunk
+// when split-KV is forced).  Co-running CTAs sweep the same K/V tiles at the same time, so each tile is fetched from
+// HBM once and then hit in L2.  See make_balanced() for the default plan.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <functional>
 #include <numeric>
@@ -100,6 +100,136 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
     heap.push(s);
   }
   c.ideal = total / n_cta;
+  c.objective = c.makespan + kPartialCost * c.n_slots / n_cta;
+}
+
+// Balanced candidate ("whole rows in lock step, then a cut tail").  A row is one (stream, head, 256-row query block)
+// over the stream's whole key range.  Rows are taken in locality order and handed whole to the queue that frees up
+// first, as long as that queue stays within the target (total cost / queues): with equal rows this is round-robin,
+// so the queues of a wave sweep the same (stream, head) K/V tiles at the same time and each tile is read from HBM
+// once.  Rows that no longer fit whole form the tail: their key ranges are laid end to end and dealt out in pieces
+// that fill every queue up to the target (no piece shorter than kMinPiece tiles), so all queues end together and only
+// tail rows produce split-KV partials.  (Cutting every queue's share out of one line - plain stream-K - balances as
+// well but de-synchronises the sweeps: measured 17 % slower on BASELINE config 5, its K/V working set leaving L2.)
+constexpr int32_t kMinPiece = 4;
+constexpr double kTileCost1 = 1.3; // one 128-key tile against a single query tile (the softmax chain, not the MMAs, bounds it)
+
+struct Row {
+  int32_t oi, head, qb, q_rows, tile0, tiles;
+  double tc;
+};
+
+void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevStream> &ds, int32_t n_heads, int32_t n_cta,
+                   double target_scale, Candidate &c) {
+  c = Candidate();
+  std::vector<Row> rows;
+  double total = 0;
+  for (size_t oi = 0; oi < order.size(); ++oi) {
+    const StreamGeom &g = order[oi];
+    const DevStream &s = ds[g.idx];
+    for (int32_t h = 0; h < n_heads; ++h)
+      for (int32_t qb = 0; qb < g.q_blocks; ++qb) {
+        Row r;
+        r.oi = (int32_t)oi;
+        r.head = h;
+        r.qb = qb;
+        r.q_rows = std::min(kItemRows, s.q_len - qb * kItemRows);
+        r.tile0 = g.tile0;
+        r.tiles = g.tiles;
+        r.tc = r.q_rows > kTileM ? kTileCost : kTileCost1;
+        total += r.tc * r.tiles + kItemOverhead;
+        rows.push_back(r);
+      }
+  }
+  const double target = target_scale * (total / n_cta) + kItemOverhead;
+  std::vector<double> load((size_t)n_cta, 0.0);
+  auto emit = [&](const Row &r, int32_t tb, int32_t take, int32_t cta) {
+    const DevStream &s = ds[order[r.oi].idx];
+    DevItem it{};
+    it.q_row0 = s.q_row0 + r.qb * kItemRows;
+    it.q_rows = r.q_rows;
+    it.head = r.head;
+    it.pt_off = s.pt_off;
+    it.kv_tile_begin = tb;
+    it.kv_tile_end = tb + take;
+    it.pos_lo = s.pos_lo;
+    it.pos_hi = s.pos_hi;
+    it.partial_slot = -1;
+    it.stream = order[r.oi].idx;
+    c.items.push_back(it);
+    c.item_cta.push_back(cta);
+    load[cta] += r.tc * take + kItemOverhead;
+  };
+  // ---- whole rows, earliest-free queue first --------------------------------------------------------------------
+  using Slot = std::pair<double, int32_t>;
+  std::priority_queue<Slot, std::vector<Slot>, std::greater<Slot>> heap;
+  for (int32_t i = 0; i < n_cta; ++i) heap.push({0.0, i});
+  std::vector<Row> tail;
+  for (const Row &r : rows) {
+    const Slot top = heap.top();
+    if (top.first + r.tc * r.tiles + kItemOverhead <= target + 1e-9) {
+      heap.pop();
+      emit(r, r.tile0, r.tiles, top.second);
+      heap.push({load[top.second], top.second});
+    } else {
+      tail.push_back(r);
+    }
+  }
+  // ---- the tail, cut to fill the queues -------------------------------------------------------------------------
+  std::vector<int32_t> by_load((size_t)n_cta);
+  std::iota(by_load.begin(), by_load.end(), 0);
+  std::stable_sort(by_load.begin(), by_load.end(), [&](int32_t a, int32_t b) { return load[a] < load[b]; });
+  size_t ti = 0;       // current tail row
+  int32_t tb = 0, rem = 0;
+  size_t first_piece = 0;
+  auto open_row = [&]() {
+    tb = tail[ti].tile0;
+    rem = tail[ti].tiles;
+    first_piece = c.items.size();
+  };
+  auto close_row = [&]() {
+    const int32_t np = (int32_t)(c.items.size() - first_piece);
+    if (np > 1) {
+      const Row &r = tail[ti];
+      DevCombine cb{};
+      cb.q_row0 = c.items[first_piece].q_row0;
+      cb.q_rows = r.q_rows;
+      cb.head = r.head;
+      cb.slot_begin = c.n_slots;
+      cb.n_parts = np;
+      c.combines.push_back(cb);
+      for (int32_t q = 0; q < np; ++q) c.items[first_piece + q].partial_slot = c.n_slots + q;
+      c.n_slots += np;
+    }
+    ++ti;
+    if (ti < tail.size()) open_row();
+  };
+  if (!tail.empty()) open_row();
+  for (int32_t qi = 0; qi < n_cta && ti < tail.size(); ++qi) {
+    const int32_t cta = by_load[qi];
+    while (ti < tail.size()) {
+      const Row &r = tail[ti];
+      const int32_t fit = (int32_t)std::floor((target - load[cta] - kItemOverhead) / r.tc + 1e-9);
+      if (fit >= rem) {
+        emit(r, tb, rem, cta);
+        close_row();
+      } else if (fit >= kMinPiece && rem - fit >= kMinPiece) {
+        emit(r, tb, fit, cta);
+        tb += fit;
+        rem -= fit;
+        break;
+      } else {
+        break;
+      }
+    }
+  }
+  while (ti < tail.size()) { // what rounding and the minimum piece length left over: to the least loaded queue
+    const int32_t cta = (int32_t)(std::min_element(load.begin(), load.end()) - load.begin());
+    emit(tail[ti], tb, rem, cta);
+    close_row();
+  }
+  c.ideal = total / n_cta;
+  for (double v : load) c.makespan = std::max(c.makespan, v);
   c.objective = c.makespan + kPartialCost * c.n_slots / n_cta;
 }
 
@@ -233,9 +363,14 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   if (opts.force_splits > 0) {
     consider(opts.force_splits, true);
   } else {
-    const int32_t ks[] = {1, 2, 3, 4, 5, 6, 8, 10, 12, 16};
-    for (int32_t k : ks)
-      if (k <= t_max) consider(k, false);
+    consider(1, false); // no split at all: best when the rows already fill the queues evenly
+    // rounding and the minimum piece length leave queues a little short or long of the target: try a few, keep the best
+    const double scales[] = {1.0, 0.99, 1.01, 0.98, 1.02, 0.97, 1.03, 1.045, 1.06};
+    for (double sc : scales) {
+      Candidate c;
+      make_balanced(order, out.streams, shape.n_heads, out.n_cta, sc, c);
+      if (c.objective < best.objective - 1e-9) best = std::move(c);
+    }
   }
 
   // ---- emit per-CTA queues (stable: queue order = item order) ------------------------------------------------
