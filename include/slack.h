@@ -161,9 +161,10 @@ slack_status slack_profile_read(slack_ctx *ctx, double *total_ms, int32_t *n_lau
 /* ---- diagnostics (never on the data path) ---------------------------------------------------------------------- */
 /* key 0: `value` = DEVICE pointer to a [2][128][128] fp32 buffer that receives the first two S = QK^T tiles computed by
  * CTA 0 of the next tensor-core launches (NULL switches the dump off).
- * key 1: `value` = DEVICE pointer to a [3][64][8] uint32 buffer; while set, tensor-core launches use a diagnostic
+ * key 1: `value` = DEVICE pointer to a uint32 buffer of 2048 + 4 * (number of SMs) words; while set, tensor-core launches use a diagnostic
  * instantiation of the kernel that stores clock64() time stamps of CTA 0's first item (rows 0/1 = softmax of query
- * tile 0/1, row 2 = MMA issuer; second index = kv step; slots documented in csrc/attn_tc.cu).  NULL switches back to
+ * tile 0/1, row 2 = MMA issuer, row 3 = per-warp arrivals; [row][kv step < 64][8 slots], slots documented in
+ * csrc/attn_tc.cu) and, from word 2048 on, {clock start, clock end, globaltimer start, end} of every CTA.  NULL switches back to
  * the production instantiation, which contains no trace code. */
 slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value);
 /* Every in-kernel barrier wait is bounded; a wait that times out records {0xDEAD, block<<32|thread, tag<<32|parity, 0}

@@ -242,7 +242,7 @@ class Context:
         self._check(self.lib.slack_debug_set(self.handle, 0, _ptr(tensor)))
 
     def debug_set_trace(self, tensor) -> None:
-        """int32/uint32 device tensor [3, 64, 8] (or None): clock trace of CTA 0's first item, see include/slack.h."""
+        """int32 device tensor of 2048 + 4 * n_sm words (or None): clock trace, see include/slack.h."""
         self._check(self.lib.slack_debug_set(self.handle, 1, _ptr(tensor)))
 
     def debug_timeout(self):

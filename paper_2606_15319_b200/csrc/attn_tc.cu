@@ -80,7 +80,7 @@ __device__ __forceinline__ ItemView view_of(const DevItem &it) {
 } // namespace
 
 // kTrace: diagnostic build that records clock64() time stamps of CTA 0's first item into p.dbg_t (slack_debug_set key 1):
-// [role 0/1 = softmax tile 0/1, 2 = MMA issuer][kv step < 64][8 slots].  The production instantiation has no trace code.
+// [role 0/1 = softmax tile 0/1, 2 = MMA issuer, 3 = per-warp arrivals][kv step < 64][8 slots], then per-CTA spans.  The production instantiation has no trace code.
 #define SLACK_TRACE(role, step, slot)                                                                      \
   if constexpr (kTrace) {                                                                                  \
     if (blockIdx.x == 0 && k == item_begin && (step) < 64 && (threadIdx.x & ((role) == 2 ? 31 : 127)) == 0)                    \
@@ -138,6 +138,14 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 
   const int H = p.n_heads;
   const int P = 1 << p.page_log2;
+  if constexpr (kTrace) { // per-CTA span: words [2048 + 4*cta .. +3] = {clock start, clock end, globaltimer start, end}
+    if (threadIdx.x == 0) {
+      unsigned long long gt;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+      p.dbg_t[2048 + 4 * blockIdx.x + 0] = (uint32_t)clock64();
+      p.dbg_t[2048 + 4 * blockIdx.x + 2] = (uint32_t)gt;
+    }
+  }
 
   if (warp < 4) {
     setmaxnreg_dec<80>();
@@ -495,6 +503,14 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
   // ---------------- teardown ----------------
   tc_fence_before();
   __syncthreads();
+  if constexpr (kTrace) {
+    if (threadIdx.x == 0) {
+      unsigned long long gt;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+      p.dbg_t[2048 + 4 * blockIdx.x + 1] = (uint32_t)clock64();
+      p.dbg_t[2048 + 4 * blockIdx.x + 3] = (uint32_t)gt;
+    }
+  }
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, 512);

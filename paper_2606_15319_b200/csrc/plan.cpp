@@ -27,7 +27,7 @@ struct StreamGeom {
 };
 
 constexpr double kTileCost = 2.0;      // one 128-key tile against a 256-row item (two MMA tile pairs)
-constexpr double kItemOverhead = 5.0;  // pipeline fill/drain + epilogue, in the same unit
+constexpr double kItemOverhead = 9.0;  // pipeline fill/drain + epilogue: measured ~15k cycles = 4.4 steps of 3400 (per-CTA span fit)
 constexpr double kPartialCost = 3.0;   // extra epilogue traffic + combine work per partial slot
 
 struct Candidate {
@@ -112,7 +112,7 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
 // tail rows produce split-KV partials.  (Cutting every queue's share out of one line - plain stream-K - balances as
 // well but de-synchronises the sweeps: measured 17 % slower on BASELINE config 5, its K/V working set leaving L2.)
 constexpr int32_t kMinPiece = 4;
-constexpr double kTileCost1 = 1.3; // one 128-key tile against a single query tile (the softmax chain, not the MMAs, bounds it)
+constexpr double kTileCost1 = 1.55; // one 128-key tile against a single query tile: measured 2620 vs 3400 cycles (the chain bounds it)
 
 struct Row {
   int32_t oi, head, qb, q_rows, tile0, tiles;

@@ -48,6 +48,34 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int tag
     }
   }
 }
+// Same contract as mbar_wait, but polls with the non-suspending test_wait: for the MMA issuer, whose barriers are
+// usually complete (or about to be) when it looks, a suspended try_wait costs hundreds of cycles on the tensor pipe's
+// critical path.
+__device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity, int tag, unsigned long long *dbg) {
+  uint32_t spins = 0;
+  while (!mbar_test_wait(bar, parity)) {
+    if (++spins > (1u << 26)) {
+      if (dbg) {
+        dbg[0] = 0xDEADull;
+        dbg[1] = ((unsigned long long)blockIdx.x << 32) | (unsigned long long)threadIdx.x;
+        dbg[2] = ((unsigned long long)(uint32_t)tag << 32) | parity;
+      }
+      __threadfence_system();
+      __trap();
+    }
+  }
+}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
