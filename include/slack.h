@@ -46,7 +46,7 @@ typedef enum {
   SLACK_OK = 0,
   SLACK_EINVAL = 1,       /* malformed descriptors: negative lengths, base >= page_size, short page table, page id out of
                              range, a physical page owned twice in the batch, misaligned (<16 B) pointer, NULL argument */
-  SLACK_EUNSUPPORTED = 2, /* valid but not built: sink_len != 0, head_dim not in {64,128}, page_size not a power of two >= 16 */
+  SLACK_EUNSUPPORTED = 2, /* valid but not built: head_dim not in {64,128}, page_size not a power of two >= 16 */
   SLACK_ENOMEM = 3,       /* host or device allocation failed, or workspace_bytes too small */
   SLACK_ECUDA = 4,        /* a CUDA runtime/driver call failed, or the context has no device */
   SLACK_ESTALE_PLAN = 5   /* plan does not match the pool shape / dtype passed with it */
@@ -73,7 +73,9 @@ typedef struct {
   int32_t cache_len;         /* Lc: tokens of earlier chunks held for this stream                               */
   int32_t base;              /* slot of logical token 0 inside page_table[0]; 0 <= base < page_size             */
   int32_t window;            /* Wt: max visible keys INCLUDING the own chunk; 0 = unlimited              */
-  int32_t sink_len;          /* reserved ("sink + local"); must be 0, else SLACK_EUNSUPPORTED             */
+  int32_t sink_len;          /* "sink + local": the first sink_len tokens stay visible when the window has
+                                moved past them: visible = [0, sink) U [max(sink, lo), n); 0 = no sink; their pages
+                                must still be listed in page_table                                                */
   int32_t n_table_pages;     /* >= ceil((base + Lc + Lq) / page_size)                                           */
   const int32_t *page_table; /* HOST: logical page -> physical page id in [0, n_pages)                          */
 } slack_stream;
@@ -101,6 +103,9 @@ typedef struct {
   int32_t kv_tile_end;
   int32_t pos_lo;        /* visible positions [pos_lo, pos_hi) = [base + lo, base + n)                           */
   int32_t pos_hi;
+  int32_t sink_tiles;    /* tiles of the sink [base, sink_pos_hi) visited BEFORE the window tiles (0: none; only the
+                            first piece of a split row carries them), starting at tile base / 128                  */
+  int32_t sink_pos_hi;   /* base + sink_len when the item visits sink tiles, else base                            */
   int32_t partial_slot;  /* -1: writes `out` directly; >= 0: writes workspace slot (split-KV), combined afterwards */
   int32_t cta;           /* CTA (0..sm_count-1) whose queue holds this item                                      */
 } slack_work_item;

@@ -313,6 +313,8 @@ int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, i
     w.kv_tile_end = d.kv_tile_end;
     w.pos_lo = d.pos_lo;
     w.pos_hi = d.pos_hi;
+    w.sink_tiles = d.sink_tiles;
+    w.sink_pos_hi = d.sink_hi;
     w.partial_slot = d.partial_slot;
     w.cta = hp.item_cta[i];
   }

@@ -48,7 +48,11 @@ attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k_pool, const T 
     acc[e] = 0.f;
   }
   float m = -INFINITY, l = 0.f;
-  for (int pos = s.pos_lo; pos < s.pos_hi; ++pos) {
+  // visible positions: the sink [base, sink_hi) (empty unless the window has left it behind), then [pos_lo, pos_hi)
+  const int n_sink = s.sink_hi - s.base;
+  const int n_vis = n_sink + (s.pos_hi - s.pos_lo);
+  for (int t = 0; t < n_vis; ++t) {
+    const int pos = t < n_sink ? s.base + t : s.pos_lo + (t - n_sink);
     const long long page = pt[pos >> page_log2];
     const long long off = ((((page * n_heads + h) << page_log2) + (pos & page_mask)) * D) + lane * E;
     float dot = 0.f;

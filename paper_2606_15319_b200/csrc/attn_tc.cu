@@ -64,16 +64,42 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr int kEmuOf8 = SLACK_EMU_OF_8; // pairs out of every 8 whose exp2 runs on the FMA pipe instead of the MUFU
 constexpr float kRescaleThreshold = 8.0f; // skip the O rescale while the row max grew by < 2^8 (in exp2 units)
 
+// Key-tile steps of an item: ns sink tiles ("sink + local"; first piece of a row only) and then the window tiles
+// [tb, te).  Step j visits tile_of(j); its visible positions are [lo_of(j), hi_of(j)).
 struct ItemView {
-  int tb, te, T, nq;
+  int tb, te, T, nq, ns, st0, s_lo, s_hi, w_lo, w_hi;
+  __device__ __forceinline__ int tile_of(int j) const { return j < ns ? st0 + j : tb + (j - ns); }
+  __device__ __forceinline__ int lo_of(int j) const { return j < ns ? s_lo : w_lo; }
+  __device__ __forceinline__ int hi_of(int j) const { return j < ns ? s_hi : w_hi; }
 };
 
 __device__ __forceinline__ ItemView view_of(const DevItem &it) {
   ItemView v;
   v.tb = it.kv_tile_begin;
   v.te = it.kv_tile_end;
-  v.T = v.te - v.tb;
+  v.ns = it.sink_tiles;
+  v.st0 = it.sink_tile0;
+  v.s_lo = it.sink_lo;
+  v.s_hi = it.sink_hi;
+  v.w_lo = it.pos_lo;
+  v.w_hi = it.pos_hi;
+  v.T = v.ns + v.te - v.tb;
   v.nq = it.q_rows > kTileM ? 2 : 1;
+  return v;
+}
+// the same view with every field broadcast from lane 0 (warp-uniform for the compiler)
+__device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
+  ItemView v = view_of(it);
+  v.tb = uni(v.tb);
+  v.te = uni(v.te);
+  v.ns = uni(v.ns);
+  v.st0 = uni(v.st0);
+  v.s_lo = uni(v.s_lo);
+  v.s_hi = uni(v.s_hi);
+  v.w_lo = uni(v.w_lo);
+  v.w_hi = uni(v.w_hi);
+  v.T = uni(v.T);
+  v.nq = uni(v.nq);
   return v;
 }
 
@@ -156,10 +182,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       int n_item = 0;
       for (int k = item_begin; k < item_end; ++k, ++n_item) {
         const DevItem it = p.items[k];
-        ItemView v = view_of(it);
-        v.tb = uni(v.tb);
-        v.te = uni(v.te);
-        v.nq = uni(v.nq);
+        const ItemView v = uniform_view_of(it);
         const int head = uni(it.head), q_row0 = uni(it.q_row0), pt_off = uni(it.pt_off);
         mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
         if (elect_one()) {
@@ -170,14 +193,14 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                           q_row0 + i * kTileM);
         }
         __syncwarp();
-        for (int t0 = v.tb; t0 < v.te; t0 += 32) {
-          const int my_t = t0 + lane;
+        for (int j0 = 0; j0 < v.T; j0 += 32) { // 32 steps at a time: each lane looks up the page of one step's tile
+          const int my_j = j0 + lane;
           int my_page = 0;
-          if (my_t < v.te) my_page = __ldg(p.page_tables + pt_off + ((my_t * kTileN) >> p.page_log2));
-          const int cnt = min(32, v.te - t0);
+          if (my_j < v.T) my_page = __ldg(p.page_tables + pt_off + ((v.tile_of(my_j) * kTileN) >> p.page_log2));
+          const int cnt = min(32, v.T - j0);
           for (int j = 0; j < cnt; ++j) {
             const int page = __shfl_sync(0xffffffffu, my_page, j);
-            const int row = (page * H + head) * P + (((t0 + j) * kTileN) & (P - 1));
+            const int row = (page * H + head) * P + ((v.tile_of(j0 + j) * kTileN) & (P - 1));
 #pragma unroll
             for (int kv = 0; kv < 2; ++kv) {
               const uint32_t stage = ring % kStages;
@@ -226,11 +249,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       };
       for (int k = item_begin; k < item_end; ++k, ++n_item) {
         const DevItem it = p.items[k];
-        ItemView v = view_of(it);
-        v.tb = uni(v.tb);
-        v.T = uni(v.T);
-        v.nq = uni(v.nq);
-        const int pos_lo = uni(it.pos_lo), pos_hi = uni(it.pos_hi);
+        const ItemView v = uniform_view_of(it);
         const uint32_t r0 = ring;
         mbar_wait(bar(BAR_Q_FULL), (uint32_t)(n_item & 1), 200, dbg);
         {
@@ -258,9 +277,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           SLACK_TRACE(2, j, 1);
           {
             // masked key rows of V must be zero: P is 0 there, but 0 * NaN/Inf garbage would poison O
-            const int tile = v.tb + j;
-            const int c_lo = max(0, pos_lo - tile * kTileN);
-            const int c_hi = min(kTileN, pos_hi - tile * kTileN);
+            const int tile = v.tile_of(j);
+            const int c_lo = max(0, v.lo_of(j) - tile * kTileN);
+            const int c_hi = min(kTileN, v.hi_of(j) - tile * kTileN);
             if (c_lo > 0 || c_hi < kTileN) {
               const int n_zero = c_lo + (kTileN - c_hi);
               const uint32_t base = sKV + stage_v * kTileBytes;
@@ -341,9 +360,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         }
         tmem_wait_ld();
         SLACK_TRACE(i, j, 2);
-        const int tile = v.tb + j;
-        const int c_lo = max(0, it.pos_lo - tile * kTileN);
-        const int c_hi = min(kTileN, it.pos_hi - tile * kTileN);
+        const int tile = v.tile_of(j);
+        const int c_lo = max(0, v.lo_of(j) - tile * kTileN);
+        const int c_hi = min(kTileN, v.hi_of(j) - tile * kTileN);
         if (c_lo > 0 || c_hi < kTileN) {
 #pragma unroll
           for (int e = 0; e < 128; ++e) s[e] = (e >= c_lo && e < c_hi) ? s[e] : -INFINITY;

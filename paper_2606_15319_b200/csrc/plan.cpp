@@ -22,9 +22,18 @@ namespace {
 
 struct StreamGeom {
   int32_t idx;
-  int32_t tile0, tiles;   // position-tile range
+  int32_t tile0, tiles;   // position-tile range of the window part [pos_lo, pos_hi)
   int32_t q_blocks;       // ceil(q_len / 256)
+  int32_t sink_tile0, sink_tiles; // tiles holding the visible sink positions [base, sink_hi) (0 tiles: no sink)
 };
+
+// the sink part of a row rides with the row's first piece
+void set_sink(DevItem &it, const StreamGeom &g, const DevStream &s, bool first_piece) {
+  it.sink_lo = s.base;
+  it.sink_hi = first_piece ? s.sink_hi : s.base;
+  it.sink_tile0 = g.sink_tile0;
+  it.sink_tiles = first_piece ? g.sink_tiles : 0;
+}
 
 constexpr double kTileCost = 2.0;      // one 128-key tile against a 256-row item (two MMA tile pairs)
 constexpr double kItemOverhead = 9.0;  // pipeline fill/drain + epilogue: measured ~15k cycles = 4.4 steps of 3400 (per-CTA span fit)
@@ -78,6 +87,7 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
           it.pos_hi = s.pos_hi;
           it.partial_slot = (np > 1) ? slot0 + qb * np + p : -1;
           it.stream = g.idx;
+          set_sink(it, g, s, p == 0);
           c.items.push_back(it);
         }
       }
@@ -90,7 +100,7 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
   c.item_cta.resize(c.items.size());
   double total = 0;
   for (size_t i = 0; i < c.items.size(); ++i) {
-    const double cost = kTileCost * (c.items[i].kv_tile_end - c.items[i].kv_tile_begin) + kItemOverhead;
+    const double cost = kTileCost * (c.items[i].kv_tile_end - c.items[i].kv_tile_begin + c.items[i].sink_tiles) + kItemOverhead;
     Slot s = heap.top();
     heap.pop();
     c.item_cta[i] = s.second;
@@ -115,7 +125,7 @@ constexpr int32_t kMinPiece = 4;
 constexpr double kTileCost1 = 1.55; // one 128-key tile against a single query tile: measured 2620 vs 3400 cycles (the chain bounds it)
 
 struct Row {
-  int32_t oi, head, qb, q_rows, tile0, tiles;
+  int32_t oi, head, qb, q_rows, tile0, tiles, sink_tiles;
   double tc;
 };
 
@@ -136,8 +146,9 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
         r.q_rows = std::min(kItemRows, s.q_len - qb * kItemRows);
         r.tile0 = g.tile0;
         r.tiles = g.tiles;
+        r.sink_tiles = g.sink_tiles;
         r.tc = r.q_rows > kTileM ? kTileCost : kTileCost1;
-        total += r.tc * r.tiles + kItemOverhead;
+        total += r.tc * (r.tiles + r.sink_tiles) + kItemOverhead;
         rows.push_back(r);
       }
   }
@@ -156,9 +167,11 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
     it.pos_hi = s.pos_hi;
     it.partial_slot = -1;
     it.stream = order[r.oi].idx;
+    const bool first_piece = tb == r.tile0;
+    set_sink(it, order[r.oi], s, first_piece);
     c.items.push_back(it);
     c.item_cta.push_back(cta);
-    load[cta] += r.tc * take + kItemOverhead;
+    load[cta] += r.tc * (take + (first_piece ? r.sink_tiles : 0)) + kItemOverhead;
   };
   // ---- whole rows, earliest-free queue first --------------------------------------------------------------------
   using Slot = std::pair<double, int32_t>;
@@ -167,7 +180,7 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
   std::vector<Row> tail;
   for (const Row &r : rows) {
     const Slot top = heap.top();
-    if (top.first + r.tc * r.tiles + kItemOverhead <= target + 1e-9) {
+    if (top.first + r.tc * (r.tiles + r.sink_tiles) + kItemOverhead <= target + 1e-9) {
       heap.pop();
       emit(r, r.tile0, r.tiles, top.second);
       heap.push({load[top.second], top.second});
@@ -209,7 +222,7 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
     const int32_t cta = by_load[qi];
     while (ti < tail.size()) {
       const Row &r = tail[ti];
-      const int32_t fit = (int32_t)std::floor((target - load[cta] - kItemOverhead) / r.tc + 1e-9);
+      const int32_t fit = (int32_t)std::floor((target - load[cta] - kItemOverhead) / r.tc + 1e-9) - (tb == r.tile0 ? r.sink_tiles : 0);
       if (fit >= rem) {
         emit(r, tb, rem, cta);
         close_row();
@@ -277,9 +290,9 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
       snprintf(buf, sizeof buf, "stream %d: base %d outside [0, page_size)", i, s.base);
       return fail(SLACK_EINVAL, buf);
     }
-    if (s.sink_len != 0) {
-      snprintf(buf, sizeof buf, "stream %d: sink_len != 0 is reserved", i);
-      return fail(SLACK_EUNSUPPORTED, buf);
+    if (s.sink_len < 0) {
+      snprintf(buf, sizeof buf, "stream %d: negative sink_len", i);
+      return fail(SLACK_EINVAL, buf);
     }
     const int64_t n = (int64_t)s.cache_len + s.q_len;
     if ((int64_t)s.base + n > (int64_t)INT32_MAX / 2 || row + s.q_len > (int64_t)INT32_MAX / 2)
@@ -298,9 +311,13 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     d.q_len = s.q_len;
     d.cache_len = s.cache_len;
     d.base = s.base;
-    const int64_t lo = (s.window > 0) ? std::max<int64_t>(0, n - s.window) : 0;
+    // visible tokens = [0, sink) U [max(sink, lo), n) ("sink + local"); one range when they touch or overlap
+    int64_t lo = (s.window > 0) ? std::max<int64_t>(0, n - s.window) : 0;
+    const int64_t sink = std::min<int64_t>(s.sink_len, n);
+    if (lo <= sink) lo = 0;
     d.pos_lo = (int32_t)(s.base + lo);
     d.pos_hi = (int32_t)(s.base + n);
+    d.sink_hi = (int32_t)(s.base + (lo > 0 ? sink : 0));
     d.pt_off = (int32_t)out.page_tables.size();
     d.n_table_pages = need;
     for (int32_t p = 0; p < need; ++p) {
@@ -335,9 +352,12 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     g.tile0 = d.pos_lo / kTileN;
     g.tiles = ceil_div(d.pos_hi, kTileN) - g.tile0;
     g.q_blocks = ceil_div(d.q_len, kItemRows);
+    g.sink_tile0 = d.base / kTileN;
+    g.sink_tiles = d.sink_hi > d.base ? ceil_div(d.sink_hi, kTileN) - g.sink_tile0 : 0;
     order.push_back(g);
   }
-  std::stable_sort(order.begin(), order.end(), [](const StreamGeom &a, const StreamGeom &b) { return a.tiles > b.tiles; });
+  std::stable_sort(order.begin(), order.end(),
+                   [](const StreamGeom &a, const StreamGeom &b) { return a.tiles + a.sink_tiles > b.tiles + b.sink_tiles; });
   if (order.empty()) return SLACK_OK;
 
   const int32_t t_max = order.front().tiles;

@@ -15,7 +15,10 @@ constexpr int kTileM = 128;    // query rows per MMA tile (UMMA M)
 constexpr int kTileN = 128;    // keys per KV tile (UMMA N of QK^T, K extent of PV); anchored to page slots
 constexpr int kItemRows = 256; // an item carries two query tiles that ping-pong on the tensor pipe
 
-// One planned unit of work as the kernels read it (device copy of slack_work_item plus table offsets). 48 bytes.
+// One planned unit of work as the kernels read it (device copy of slack_work_item plus table offsets). 64 bytes.
+// Key tiles are visited in the order: sink tiles [sink_tile0, sink_tile0 + sink_tiles) with visible positions
+// [sink_lo, sink_hi) ("sink + local"; only the first piece of a row carries them), then the window tiles
+// [kv_tile_begin, kv_tile_end) with visible positions [pos_lo, pos_hi).
 struct DevItem {
   int32_t q_row0;        // global row (ragged concat) of the item's first query row
   int32_t q_rows;        // valid rows, 1..256
@@ -27,9 +30,13 @@ struct DevItem {
   int32_t pos_hi;
   int32_t partial_slot;  // -1 = final output, else workspace slot
   int32_t stream;
+  int32_t sink_lo;       // = base
+  int32_t sink_hi;       // = base + sink (== sink_lo when the item has no sink tiles)
+  int32_t sink_tile0;
+  int32_t sink_tiles;
   int32_t pad0, pad1;
 };
-static_assert(sizeof(DevItem) == 48, "DevItem layout");
+static_assert(sizeof(DevItem) == 64, "DevItem layout");
 
 // One output row-block whose key range was cut: the combine kernel merges its partial slots (A4).
 struct DevCombine {
@@ -52,8 +59,10 @@ struct DevStream {
   int32_t pos_hi;   // base + n
   int32_t pt_off;
   int32_t n_table_pages;
+  int32_t sink_hi;  // visible sink positions [base, sink_hi) in front of [pos_lo, pos_hi); == base when there are none
+  int32_t pad0;
 };
-static_assert(sizeof(DevStream) == 32, "DevStream layout");
+static_assert(sizeof(DevStream) == 40, "DevStream layout");
 
 // Workspace layout for split-KV partials: slot s holds kItemRows rows of head_dim fp32 (normalised partial output)
 // followed, in a second region, by kItemRows fp32 lse values.

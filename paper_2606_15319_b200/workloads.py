@@ -200,3 +200,18 @@ def small_ragged(seed: int = 11, dtype: str = "bf16", n_heads: int = 2, head_dim
     return make_workload(f"small_ragged_{dtype}", dtype=dtype, n_heads=n_heads, head_dim=head_dim,
                          page_size=page_size, q_lens=q_lens, cache_lens=cache_lens, windows=windows,
                          bases=bases, seed=seed, amp=amp, spare_pages=3)
+
+
+def sink_ragged(seed: int = 13, dtype: str = "bf16", n_heads: int = 2, head_dim: int = 128,
+                page_size: int = 128, amp: float = 0.5) -> Workload:
+    """"Sink + local" cases: windows that have moved past the sink (two visible ranges, the
+    sink ending mid-tile and sharing / not sharing a tile with the window start), a sink the window still touches
+    (one range), a sink longer than the stream, and a stream without sink in the same batch."""
+    q_lens = [300, 129, 72, 257, 128, 64]
+    cache_lens = [1517, 900, 1000, 255, 2000, 300]
+    windows = [600, 400, 300, 400, 512, 0]
+    sink_lens = [72, 200, 1, 300, 4096, 16]
+    bases = [0, 5, 77 % page_size, 1, 0, 3]
+    return make_workload(f"sink_ragged_{dtype}", dtype=dtype, n_heads=n_heads, head_dim=head_dim,
+                         page_size=page_size, q_lens=q_lens, cache_lens=cache_lens, windows=windows,
+                         bases=bases, sink_lens=sink_lens, seed=seed, amp=amp, spare_pages=3)

@@ -44,7 +44,7 @@ def test_every_declared_symbol_is_exported_and_bound():
 def test_struct_sizes_match_header():
     import ctypes as C
     assert C.sizeof(binding.CPool) == 40 and C.sizeof(binding.CStream) == 32
-    assert C.sizeof(binding.CPlanOpts) == 16 and C.sizeof(binding.CWorkItem) == 40
+    assert C.sizeof(binding.CPlanOpts) == 16 and C.sizeof(binding.CWorkItem) == 48
 
 
 def test_host_only_context_has_no_data_path(hctx):
@@ -86,8 +86,12 @@ def check_cover(w, plan, n_cta):
             continue
         n = s.cache_len + s.q_len
         lo = max(0, n - s.window) if s.window > 0 else 0
+        sink = min(getattr(s, "sink_len", 0), n)
+        if lo <= sink:                      # the window still touches the sink: one visible range
+            lo, sink = 0, 0
         pos_lo, pos_hi = s.base + lo, s.base + n
         t0, t1 = pos_lo // 128, -(-pos_hi // 128)
+        want_sink_tiles = (-(-(s.base + sink) // 128) - s.base // 128) if sink > 0 else 0
         for h in range(w.n_heads):
             covered = 0
             for qb in range(-(-s.q_len // 256)):
@@ -95,10 +99,13 @@ def check_cover(w, plan, n_cta):
                 assert parts[0]["kv_tile_begin"] == t0 and parts[-1]["kv_tile_end"] == t1
                 for a, b in zip(parts, parts[1:]):
                     assert a["kv_tile_end"] == b["kv_tile_begin"]
-                for p in parts:
+                for pi, p in enumerate(parts):
                     assert (p["pos_lo"], p["pos_hi"]) == (pos_lo, pos_hi)
                     assert p["q_rows"] == min(256, s.q_len - qb * 256)
                     assert (p["partial_slot"] >= 0) == (len(parts) > 1)
+                    # the sink rides with the first piece of the row only
+                    assert p["sink_tiles"] == (want_sink_tiles if pi == 0 else 0)
+                    assert p["sink_pos_hi"] == (s.base + sink if pi == 0 else s.base)
                 covered += parts[0]["q_rows"]
             assert covered == s.q_len
         row0 += s.q_len
@@ -107,8 +114,9 @@ def check_cover(w, plan, n_cta):
 
 @pytest.mark.parametrize("splits", [0, 1, 2, 5])
 @pytest.mark.parametrize("n_cta", [1, 7, 148])
-def test_plan_cover_small(hctx, splits, n_cta):
-    w = W.small_ragged()
+@pytest.mark.parametrize("make", [W.small_ragged, W.sink_ragged])
+def test_plan_cover_small(hctx, splits, n_cta, make):
+    w = make()
     plan = hctx.slack_plan(_pool(w), w.streams, sm_count=n_cta, force_splits=splits)
     assert plan.kernel_kind == 0
     check_cover(w, plan, n_cta)
@@ -171,7 +179,7 @@ def test_plan_rejects_malformed_descriptors(hctx):
     _expect(hctx, E, w, mutate=lambda s: s[0].page_table.__setitem__(0, w.n_pages))
     _expect(hctx, E, w, mutate=lambda s: s[0].page_table.__setitem__(0, -1))
     _expect(hctx, E, w, mutate=lambda s: s[1].page_table.__setitem__(0, int(s[0].page_table[0])))   # page owned twice
-    _expect(hctx, U, w, mutate=lambda s: setattr(s[0], "sink_len", 4))
+    _expect(hctx, E, w, mutate=lambda s: setattr(s[0], "sink_len", -4))
     _expect(hctx, U, w, pool=_pool(w, head_dim=96))
     _expect(hctx, U, w, pool=_pool(w, page_size=48))
     _expect(hctx, U, w, pool=_pool(w, page_size=8))

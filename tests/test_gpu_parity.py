@@ -81,6 +81,23 @@ def test_small_ragged_tensor_core(ctx, page_size, splits):
     assert res["kind"] == 0
 
 
+# ------------------------------------------------------------------------------------------------ sink + local
+@pytest.mark.parametrize("page_size", [128, 256])
+@pytest.mark.parametrize("splits", [0, 1, 3])
+def test_sink_plus_local_window_tensor_core(ctx, page_size, splits):
+    """Visible keys = [0, sink) U [max(sink, lo), n): the sink tiles are visited before the window tiles of the first
+    piece of every row; sink ends mid-tile, shares a tile with the window start, or is absorbed by the window."""
+    res, *_ = run_case(ctx, W.sink_ragged(page_size=page_size), force_splits=splits)
+    assert res["kind"] == 0
+
+
+def test_sink_plus_local_window_simt(ctx):
+    res, *_ = run_case(ctx, W.sink_ragged(dtype="f32", head_dim=64, page_size=16), tol=(1e-5, 1e-5))
+    assert res["kind"] == 1
+    res, *_ = run_case(ctx, W.sink_ragged(), force_simt=1)
+    assert res["kind"] == 1
+
+
 def test_small_ragged_simt_bf16_and_small_pages(ctx):
     res, *_ = run_case(ctx, W.small_ragged(page_size=32))
     assert res["kind"] == 1          # page_size < 128 is served by the SIMT path
