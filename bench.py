@@ -204,7 +204,7 @@ def run_reference(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per attention-kernel launch from the committed `ncu --set full`
 # capture (profiles/): filled per workload once measured, else null.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"cfg2": 216167680}   # profiles/r01_ncu_full_cfg2.md: 195.06 MB read + 21.11 MB written per launch
 
 
 def run_ours(args):
