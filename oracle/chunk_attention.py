@@ -25,6 +25,14 @@ Definition; for stream s, head h, with n = Lc + Lq:
 Token t of a stream lives at physical page page_table[(base+t) // P], slot (base+t) % P of a pool
 laid out [n_pages][H][P][D] (the token->slot rule of include/slack.h).
 
+Block-sparse variant (PAPER.md P:88 knob (2) "skips nonselected attention blocks
+with sparse masks ... controlled by attention sparsity rho", rho in {0,.6,.7,.8,.9} P:568, selection
+rule from Light Forcing [39] P:319 - the rule is NOT in the paper, so the mask is an INPUT here):
+    query block  qb = i // block_q            (i = chunk-local query row)
+    key block    kb = (base + t) // block_k   (position of key token t in the stream's page-table space)
+    t is used iff it is visible (above) AND mask[h, qb, kb]
+    out_i = softmax over the used keys; a row with no used key has out_i = 0 and lse_i = -inf.
+
 Since attention is a *defined* function the oracle is that definition written out: gather, one
 matmul, a max-subtracted exp, one matmul, a division - in fp64, no tiling over keys, no online
 softmax, no splits.  Query rows are processed in blocks of <= `row_block` rows only to bound
@@ -33,6 +41,10 @@ memory (rows are independent, so this changes no row's arithmetic).
 Pins (tests/test_oracle_pins.py): pure-Python brute force, closed forms (V=1, K=0 mean, single key,
 one-hot V, logit shift), torch SDPA fp64, dense block-causal masked attention over the whole
 sequence, page permutation invariance, NaN poisoning of unowned slots, scipy logsumexp, LSE merge.
+Block-sparse pins (tests/test_oracle_sparse_pins.py): all-ones mask == dense, pure-Python brute force
+with tiny blocks, torch SDPA fp64 with an element-wise boolean mask, K=0 closed form (mean of V over the
+used keys, base/window swept), disjoint-mask LSE merge == union mask, bits of invisible blocks ignored,
+empty rows.
 The paper prints no numeric example for this path, so no paper-valued fixture exists.
 """
 from __future__ import annotations
@@ -119,14 +131,40 @@ def attend_rows(q_rows: np.ndarray, k: np.ndarray, v: np.ndarray, scale: float):
     return out, lse
 
 
+def _sparse_stream(k_pool, v_pool, s, toks, sel, q, row0, scale, dtype, mask, block_q, block_k, out, lse) -> None:
+    """Block-sparse rows of one stream: for every head and query block, softmax over the visible keys whose
+    key block is selected (header; P:88 knob (2)).  Rows of one query block share their key set."""
+    n_heads = q.shape[1]
+    key_block = (s.base + toks) // block_k                 # key block of every visible token
+    assert mask.shape[0] == n_heads and mask.shape[1] >= -(-s.q_len // block_q) and mask.shape[2] > int(key_block.max())
+    for h in range(n_heads):
+        for qb in np.unique(sel // block_q):
+            r = sel[sel // block_q == qb]
+            used = toks[mask[h, qb, key_block]]            # visible AND selected
+            if used.size == 0:
+                out[row0 + r, h, :] = 0.0
+                lse[h, row0 + r] = -np.inf
+                continue
+            kh = to_f64(np.ascontiguousarray(gather_kv(k_pool, s, used)[:, h, :]), dtype)
+            vh = to_f64(np.ascontiguousarray(gather_kv(v_pool, s, used)[:, h, :]), dtype)
+            qh = to_f64(np.ascontiguousarray(q[row0 + r, h, :]), dtype)
+            o, l = attend_rows(qh, kh, vh, scale)
+            out[row0 + r, h, :] = o
+            lse[h, row0 + r] = l
+
+
 def chunk_attention(k_pool: np.ndarray, v_pool: np.ndarray, streams: Sequence, q: np.ndarray,
                     scale: float, dtype: str, row_block: int = 512,
-                    rows: Optional[Sequence[Optional[np.ndarray]]] = None):
+                    rows: Optional[Sequence[Optional[np.ndarray]]] = None,
+                    block_masks: Optional[Sequence[Optional[np.ndarray]]] = None,
+                    block_q: int = 256, block_k: int = 128):
     """Ragged chunk attention for a batch of streams; precondition: own chunk already appended.
 
     q: [sum Lq, H, D] storage dtype.  Returns (out fp64 [sum Lq, H, D], lse fp64 [H, sum Lq]).
     `rows`: optional per-stream arrays of chunk-local query rows to compute (others stay NaN) - rows
     are independent, so a sampled row is exact (used at full size).
+    `block_masks`: optional per-stream boolean arrays [H, ceil(Lq/block_q), >= ceil((base+n)/block_k)]
+    (None = dense for that stream): the block-sparse variant of the header (P:88 knob (2)).
     """
     total_q, n_heads, head_dim = q.shape
     out = np.full((total_q, n_heads, head_dim), np.nan, dtype=np.float64)
@@ -137,7 +175,10 @@ def chunk_attention(k_pool: np.ndarray, v_pool: np.ndarray, streams: Sequence, q
             continue
         toks = visible_tokens(s)
         sel = np.arange(s.q_len) if rows is None or rows[si] is None else np.asarray(rows[si], dtype=np.int64)
-        if sel.size:
+        if sel.size and block_masks is not None and block_masks[si] is not None:
+            _sparse_stream(k_pool, v_pool, s, toks, sel, q, row0, scale, dtype, np.asarray(block_masks[si], dtype=bool),
+                           block_q, block_k, out, lse)
+        elif sel.size:
             k_all = gather_kv(k_pool, s, toks)          # [Lk, H, D] storage
             v_all = gather_kv(v_pool, s, toks)
             for h in range(n_heads):

@@ -215,3 +215,76 @@ def sink_ragged(seed: int = 13, dtype: str = "bf16", n_heads: int = 2, head_dim:
     return make_workload(f"sink_ragged_{dtype}", dtype=dtype, n_heads=n_heads, head_dim=head_dim,
                          page_size=page_size, q_lens=q_lens, cache_lens=cache_lens, windows=windows,
                          bases=bases, sink_lens=sink_lens, seed=seed, amp=amp, spare_pages=3)
+
+
+# ----------------------------------------------------------------------------------------------
+# block-sparse masks (P:88 knob (2), rho in {0,.6,.7,.8,.9} P:568)
+# ----------------------------------------------------------------------------------------------
+# Geometry of the mask INPUT as include/slack.h publishes it: one bit per (head, 256-row query block, 128-position key
+# block); key block kb covers positions [128 kb, 128 kb + 128) of the stream's page-table space (position = base + token).
+MASK_BLOCK_Q = 256
+MASK_BLOCK_K = 128
+
+
+def visible_key_blocks(s: StreamSpec, block_k: int = MASK_BLOCK_K) -> np.ndarray:
+    """Indices of the key blocks that hold at least one visible position of the stream (sink range, then window range)."""
+    n = s.cache_len + s.q_len
+    lo = max(0, n - s.window) if s.window > 0 else 0
+    sink = min(s.sink_len, n)
+    lo = max(lo, sink)
+    blocks = set()
+    for a, b in ((0, sink), (lo, n)):
+        if b > a:
+            blocks.update(range((s.base + a) // block_k, (s.base + b - 1) // block_k + 1))
+    return np.array(sorted(blocks), dtype=np.int64)
+
+
+def random_block_masks(w: Workload, sparsity: float, seed: int = 0, block_q: int = MASK_BLOCK_Q,
+                       block_k: int = MASK_BLOCK_K, keep_last: bool = True) -> List[Optional[np.ndarray]]:
+    """Seeded stand-in for a block-selection rule (the paper's is Light Forcing's [39], not available): per
+    stream a boolean array [H, ceil(Lq/block_q), ceil((base+n)/block_k)]; for every (head, query block) a fraction
+    `sparsity` (rounded) of the VISIBLE key blocks is dropped uniformly at random.  With keep_last the last visible block
+    (it holds the end of the own chunk) is always kept, so no row is left without a key."""
+    rng = np.random.default_rng(seed + 31)
+    masks: List[Optional[np.ndarray]] = []
+    for s in w.streams:
+        if s.q_len == 0:
+            masks.append(None)
+            continue
+        n_qb = -(-s.q_len // block_q)
+        n_kb = -(-(s.base + s.cache_len + s.q_len) // block_k)
+        vis = visible_key_blocks(s, block_k)
+        m = np.zeros((w.n_heads, n_qb, n_kb), dtype=bool)
+        n_drop = int(round(sparsity * vis.size))
+        if keep_last:
+            n_drop = min(n_drop, vis.size - 1)
+        for h in range(w.n_heads):
+            for qb in range(n_qb):
+                cand = vis[:-1] if keep_last else vis
+                drop = rng.choice(cand, size=min(n_drop, cand.size), replace=False) if n_drop > 0 else np.array([], dtype=np.int64)
+                m[h, qb, vis] = True
+                m[h, qb, drop] = False
+        masks.append(m)
+    return masks
+
+
+def pack_block_masks(w: Workload, masks: Sequence[Optional[np.ndarray]], block_q: int = MASK_BLOCK_Q,
+                     block_k: int = MASK_BLOCK_K) -> np.ndarray:
+    """The mask in the layout include/slack.h asks for: uint32 [sum_s ceil(Lq_s/block_q)][H][words], bit (kb % 32) of
+    word kb // 32 = key block kb; rows of a stream follow each other in stream order; a None mask packs as all ones."""
+    n_kb_max = max([-(-(s.base + s.cache_len + s.q_len) // block_k) for s in w.streams] + [1])
+    words = -(-n_kb_max // 32)
+    rows = []
+    for s, m in zip(w.streams, masks):
+        n_qb = -(-s.q_len // block_q)
+        if n_qb == 0:
+            continue
+        bits = np.ones((n_qb, w.n_heads, words * 32), dtype=bool)
+        if m is not None:
+            bits[:] = False
+            bits[:, :, :m.shape[2]] = np.transpose(m[:, :n_qb, :], (1, 0, 2))
+        packed = np.packbits(bits.reshape(n_qb, w.n_heads, words, 32), axis=-1, bitorder="little")
+        rows.append(packed.reshape(n_qb, w.n_heads, words, 4).view("<u4")[..., 0])
+    if not rows:
+        return np.zeros((0, w.n_heads, words), dtype=np.uint32)
+    return np.ascontiguousarray(np.concatenate(rows, axis=0), dtype=np.uint32)
