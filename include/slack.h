@@ -152,6 +152,29 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
                                    void *out, float *lse, float scale, void *workspace, size_t workspace_bytes,
                                    void *cuda_stream);
 
+/* ---- A3, block-sparse variant -------------------------------------------------------------- */
+/* PAPER.md P:88 knob (2): "skips nonselected attention blocks with sparse masks", controlled by the attention sparsity
+ * rho in {0, .6, .7, .8, .9}.  The block-SELECTION rule is Light Forcing's and not part of this path:
+ * the mask is an input.  Semantics: query row i of a stream (chunk-local) belongs to query block i / 256; key token t
+ * belongs to key block (base + t) / 128 (the 128-position key tiles of slack_work_item); row i uses key t iff t is
+ * visible (window / sink, as in slack_chunk_attention) AND its key block is selected for (query block, head).  A row
+ * that is left without any key gets out = 0 and lse = -inf.
+ * block_mask: DEVICE uint32 [slack_plan_mask_rows(plan)][n_heads][mask_words]; mask row r = the r-th 256-row query block
+ * of the batch, counting ceil(Lq/256) blocks per stream in stream order; bit (kb % 32) of word kb / 32 = key block kb;
+ * bits of blocks without a visible key are ignored; mask_words >= slack_plan_mask_min_words(plan).  The mask is read
+ * when the call executes on `cuda_stream`, so it may be produced on the device and may differ in every layer and
+ * denoising step while the plan stays valid.  workspace: >= slack_plan_sparse_workspace_bytes(plan) bytes (it holds the
+ * split-KV partials and, per planned item, the list of its selected key tiles).  Other arguments as in
+ * slack_chunk_attention.  f32 pools / force_simt plans evaluate the same definition on the SIMT kernel. */
+#define SLACK_MASK_BLOCK_Q 256
+#define SLACK_MASK_BLOCK_K 128
+slack_status slack_chunk_attention_sparse(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q,
+                                          void *out, float *lse, float scale, const uint32_t *block_mask,
+                                          int32_t mask_words, void *workspace, size_t workspace_bytes, void *cuda_stream);
+size_t slack_plan_sparse_workspace_bytes(const slack_plan_t *plan);
+int32_t slack_plan_mask_rows(const slack_plan_t *plan);      /* sum over streams of ceil(q_len / 256)                 */
+int32_t slack_plan_mask_min_words(const slack_plan_t *plan); /* ceil(max over streams of ceil((base+Lc+Lq)/128) / 32) */
+
 /* Number of kernels the last slack_chunk_attention / slack_kv_append call on this ctx launched (bench bookkeeping). */
 int32_t slack_last_launch_count(const slack_ctx *ctx);
 

@@ -64,6 +64,11 @@ SYMBOLS = {
     "slack_plan_kernel_kind": (C.c_int32, [_VP]),
     "slack_plan_get_items": (C.c_int32, [_VP, C.POINTER(CWorkItem), C.c_int32]),
     "slack_chunk_attention": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP, C.c_size_t, _VP]),
+    "slack_chunk_attention_sparse": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP, C.c_int32, _VP,
+                                              C.c_size_t, _VP]),
+    "slack_plan_sparse_workspace_bytes": (C.c_size_t, [_VP]),
+    "slack_plan_mask_rows": (C.c_int32, [_VP]),
+    "slack_plan_mask_min_words": (C.c_int32, [_VP]),
     "slack_profile_attention": (C.c_int, [_VP, C.c_int32]),
     "slack_profile_read": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_int32)]),
     "slack_debug_set": (C.c_int, [_VP, C.c_int32, _VP]),
@@ -151,6 +156,18 @@ class Plan:
         return int(load().slack_plan_workspace_bytes(self.handle))
 
     @property
+    def sparse_workspace_bytes(self) -> int:
+        return int(load().slack_plan_sparse_workspace_bytes(self.handle))
+
+    @property
+    def mask_rows(self) -> int:
+        return int(load().slack_plan_mask_rows(self.handle))
+
+    @property
+    def mask_min_words(self) -> int:
+        return int(load().slack_plan_mask_min_words(self.handle))
+
+    @property
     def num_items(self) -> int:
         return int(load().slack_plan_num_items(self.handle))
 
@@ -226,6 +243,15 @@ class Context:
         ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
         self._check(self.lib.slack_chunk_attention(self.handle, plan.handle, C.byref(pool.c), _ptr(q), _ptr(out), _ptr(lse),
                                                    C.c_float(scale), _ptr(workspace), ws_bytes, _cuda_stream(stream)))
+
+    def slack_chunk_attention_sparse(self, plan: Plan, pool: Pool, q, out, scale: float, block_mask, lse=None,
+                                     workspace=None, stream=None) -> None:
+        """block_mask: int32/uint32 device tensor [plan.mask_rows][n_heads][mask_words] (include/slack.h)."""
+        ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+        self._check(self.lib.slack_chunk_attention_sparse(self.handle, plan.handle, C.byref(pool.c), _ptr(q), _ptr(out),
+                                                          _ptr(lse), C.c_float(scale), _ptr(block_mask),
+                                                          int(block_mask.shape[-1]), _ptr(workspace), ws_bytes,
+                                                          _cuda_stream(stream)))
 
     # --- measurement ---------------------------------------------------------------------------------------------------
     def profile_attention(self, enable: bool) -> None:

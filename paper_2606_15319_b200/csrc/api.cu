@@ -294,6 +294,9 @@ void slack_plan_destroy(slack_plan_t *plan) {
 }
 
 size_t slack_plan_workspace_bytes(const slack_plan_t *plan) { return plan ? plan->hp.ws.total : 0; }
+size_t slack_plan_sparse_workspace_bytes(const slack_plan_t *plan) { return plan ? plan->hp.sparse_total : 0; }
+int32_t slack_plan_mask_rows(const slack_plan_t *plan) { return plan ? plan->hp.mask_rows : 0; }
+int32_t slack_plan_mask_min_words(const slack_plan_t *plan) { return plan ? plan->hp.mask_words_min : 0; }
 int32_t slack_plan_num_items(const slack_plan_t *plan) { return plan ? (int32_t)plan->hp.items.size() : 0; }
 int32_t slack_plan_num_partial_slots(const slack_plan_t *plan) { return plan ? plan->hp.n_partial_slots : 0; }
 int32_t slack_plan_kernel_kind(const slack_plan_t *plan) { return plan ? plan->hp.kernel_kind : -1; }
@@ -397,8 +400,13 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
 }
 
 /* ------------------------------------------------------------------------------------------------ attention */
-slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q, void *out,
-                                   float *lse, float scale, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+} // extern "C"
+
+namespace {
+// A3 + A4, dense (block_mask == NULL) or block-sparse.
+slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q, void *out,
+                            float *lse, float scale, const uint32_t *block_mask, int32_t mask_words, void *workspace,
+                            size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SLACK_EINVAL;
   ctx->last_launches = 0;
   if (!plan) return set_err(ctx, SLACK_EINVAL, "plan NULL");
@@ -411,15 +419,23 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
   if (!q || !out || !aligned(q, 16) || !aligned(out, 16)) return set_err(ctx, SLACK_EINVAL, "q / out NULL or not 16-byte aligned");
   if (!(scale > 0.f) || !(scale < 1e30f)) return set_err(ctx, SLACK_EINVAL, "scale must be a positive finite number");
   cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (block_mask) {
+    if (!aligned(block_mask, 4)) return set_err(ctx, SLACK_EINVAL, "block_mask must be 4-byte aligned");
+    if (mask_words < hp.mask_words_min) return set_err(ctx, SLACK_EINVAL, "mask_words smaller than slack_plan_mask_min_words()");
+  }
 
   if (hp.kernel_kind == 1) {
     SLACK_CUDA(ctx, launch_attn_simt(hp.dtype, q, pool->k_pool, pool->v_pool, out, lse, plan->d_streams, hp.n_streams, hp.total_q,
-                                     plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, scale, cs, &ctx->last_launches));
+                                     plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, scale, block_mask, mask_words,
+                                     cs, &ctx->last_launches));
     return SLACK_OK;
   }
 
-  if (hp.ws.total > 0) {
-    if (!workspace || workspace_bytes < hp.ws.total) return set_err(ctx, SLACK_ENOMEM, "workspace NULL or smaller than slack_plan_workspace_bytes()");
+  const size_t ws_need = block_mask ? hp.sparse_total : hp.ws.total;
+  if (ws_need > 0) {
+    if (!workspace || workspace_bytes < ws_need)
+      return set_err(ctx, SLACK_ENOMEM, block_mask ? "workspace NULL or smaller than slack_plan_sparse_workspace_bytes()"
+                                                   : "workspace NULL or smaller than slack_plan_workspace_bytes()");
     if (!aligned(workspace, 16)) return set_err(ctx, SLACK_EINVAL, "workspace must be 16-byte aligned");
   }
   if (!aligned(q, 128) || !aligned(pool->k_pool, 128) || !aligned(pool->v_pool, 128))
@@ -451,6 +467,16 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
   p.page_log2 = pl2;
   p.total_q = hp.total_q;
   p.scale = scale;
+  if (block_mask) { // the mask may change with every call: list each item's selected key-tile steps first
+    uint8_t *w8 = reinterpret_cast<uint8_t *>(workspace);
+    uint16_t *steps = reinterpret_cast<uint16_t *>(w8 + hp.sparse_steps_off);
+    int32_t *item_steps = reinterpret_cast<int32_t *>(w8 + hp.sparse_count_off);
+    SLACK_CUDA(ctx, launch_sparse_steps(plan->d_items, (int)hp.items.size(), block_mask, hp.n_heads, mask_words, steps,
+                                        item_steps, cs, &ctx->last_launches));
+    p.steps = steps;
+    p.item_steps = item_steps;
+    p.dbg_t = nullptr; // the clock-trace instantiation is dense-only
+  }
   cudaEvent_t ev_after = nullptr;
   if (ctx->prof_on) {
     while (ctx->prof_events.size() < 2 * (ctx->prof_used + 1)) {
@@ -469,6 +495,22 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
   SLACK_CUDA(ctx, launch_combine(plan->d_combines, (int)hp.combines.size(), p.ws_o, p.ws_lse, out, lse, hp.n_heads, hp.head_dim,
                                  hp.total_q, cs, &ctx->last_launches));
   return SLACK_OK;
+}
+} // namespace
+
+extern "C" {
+
+slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q, void *out,
+                                   float *lse, float scale, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  return attention_impl(ctx, plan, pool, q, out, lse, scale, nullptr, 0, workspace, workspace_bytes, cuda_stream);
+}
+
+slack_status slack_chunk_attention_sparse(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q,
+                                          void *out, float *lse, float scale, const uint32_t *block_mask, int32_t mask_words,
+                                          void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SLACK_EINVAL;
+  if (!block_mask) return set_err(ctx, SLACK_EINVAL, "block_mask NULL (use slack_chunk_attention for dense attention)");
+  return attention_impl(ctx, plan, pool, q, out, lse, scale, block_mask, mask_words, workspace, workspace_bytes, cuda_stream);
 }
 
 } // extern "C"

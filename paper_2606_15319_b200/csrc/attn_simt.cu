@@ -23,7 +23,8 @@ template <typename T, int D>
 __global__ void __launch_bounds__(kSimtThreads)
 attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k_pool, const T *__restrict__ v_pool, T *__restrict__ out,
                  float *__restrict__ lse, const DevStream *__restrict__ streams, int n_streams, int total_q,
-                 const int32_t *__restrict__ page_tables, int n_heads, int page_log2, float scale) {
+                 const int32_t *__restrict__ page_tables, int n_heads, int page_log2, float scale,
+                 const uint32_t *__restrict__ mask, int mask_words) {
   constexpr int E = D / 32; // elements per lane
   const int lane = threadIdx.x & 31;
   const long long unit = (long long)blockIdx.x * (kSimtThreads / 32) + (threadIdx.x >> 5);
@@ -47,12 +48,15 @@ attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k_pool, const T 
     qv[e] = to_f32<T>(q[((long long)row * n_heads + h) * D + lane * E + e]);
     acc[e] = 0.f;
   }
+  // block-sparse variant (P:88 knob (2)): bit t of this (256-row query block, head)'s mask row = key block t selected
+  const uint32_t *mrow = mask ? mask + ((size_t)(s.qblock0 + (row - s.q_row0) / kItemRows) * n_heads + h) * mask_words : nullptr;
   float m = -INFINITY, l = 0.f;
   // visible positions: the sink [base, sink_hi) (empty unless the window has left it behind), then [pos_lo, pos_hi)
   const int n_sink = s.sink_hi - s.base;
   const int n_vis = n_sink + (s.pos_hi - s.pos_lo);
   for (int t = 0; t < n_vis; ++t) {
     const int pos = t < n_sink ? s.base + t : s.pos_lo + (t - n_sink);
+    if (mrow != nullptr && !((__ldg(mrow + (pos / kTileN >> 5)) >> ((pos / kTileN) & 31)) & 1u)) continue;
     const long long page = pt[pos >> page_log2];
     const long long off = ((((page * n_heads + h) << page_log2) + (pos & page_mask)) * D) + lane * E;
     float dot = 0.f;
@@ -69,7 +73,7 @@ attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k_pool, const T 
     for (int e = 0; e < E; ++e) acc[e] = fmaf(pr, to_f32<T>(v_pool[off + e]), acc[e] * alpha);
     m = m_new;
   }
-  const float inv = 1.0f / l;
+  const float inv = l > 0.f ? 1.0f / l : 0.f; // no selected key (block-sparse only): out = 0, lse = -inf
 #pragma unroll
   for (int e = 0; e < E; ++e) out[((long long)row * n_heads + h) * D + lane * E + e] = from_f32<T>(acc[e] * inv);
   if (lse != nullptr && lane == 0) lse[(long long)h * total_q + row] = m + logf(l);
@@ -85,7 +89,8 @@ int ilog2(int x) {
 
 cudaError_t launch_attn_simt(int dtype, const void *q, const void *k_pool, const void *v_pool, void *out, float *lse,
                              const DevStream *d_streams, int n_streams, int total_q, const int32_t *d_page_tables,
-                             int n_heads, int head_dim, int page_size, float scale, cudaStream_t st, int *n_launched) {
+                             int n_heads, int head_dim, int page_size, float scale, const uint32_t *mask, int mask_words,
+                             cudaStream_t st, int *n_launched) {
   if (total_q == 0) return cudaSuccess;
   const long long units = (long long)total_q * n_heads;
   const int wpb = kSimtThreads / 32;
@@ -94,7 +99,7 @@ cudaError_t launch_attn_simt(int dtype, const void *q, const void *k_pool, const
 #define SLACK_SIMT_LAUNCH(T, D)                                                                                          \
   attn_simt_kernel<T, D><<<grid, kSimtThreads, 0, st>>>(reinterpret_cast<const T *>(q), reinterpret_cast<const T *>(k_pool), \
                                                         reinterpret_cast<const T *>(v_pool), reinterpret_cast<T *>(out), lse, \
-                                                        d_streams, n_streams, total_q, d_page_tables, n_heads, pl, scale)
+                                                        d_streams, n_streams, total_q, d_page_tables, n_heads, pl, scale, mask, mask_words)
   if (dtype == SLACK_F32 && head_dim == 64) SLACK_SIMT_LAUNCH(float, 64);
   else if (dtype == SLACK_F32 && head_dim == 128) SLACK_SIMT_LAUNCH(float, 128);
   else if (dtype == SLACK_BF16 && head_dim == 64) SLACK_SIMT_LAUNCH(__nv_bfloat16, 64);

@@ -15,6 +15,11 @@
 // other tile's P V and next Q K^T.  TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_i is
 // written over the first 64 columns of S_i (two bf16 per 32-bit column).
 //
+// Block-sparse variant (kSparse, PAPER.md P:88 knob (2) "skips nonselected attention blocks with
+// sparse masks"): an item visits only the key-tile steps listed for it by sparse_steps.cu (the device block mask changes
+// per layer / denoising step, the host plan does not); every role walks that list instead of 0..T-1, an item with an
+// empty list writes zeros (lse = -inf) and touches no barrier.
+//
 // Shared memory layouts (all 128-byte swizzled, as TMA writes them and as the UMMA descriptors expect them):
 //   Q tile / K tile: two 16 KB halves (d 0..63, d 64..127), each [128 rows][128 B]  -> K-major operands
 //   V tile:          same bytes; read as the MN-major B operand of P V (N = d contiguous, K = keys)
@@ -113,7 +118,7 @@ __device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
       p.dbg_t[((role) * 64 + (step)) * 8 + (slot)] = (uint32_t)clock64();                                  \
   }
 
-template <bool kTrace>
+template <bool kTrace, bool kSparse>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                const __grid_constant__ CUtensorMap tm_v) {
@@ -179,12 +184,16 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       // ============================== TMA producer ==============================
       // The whole warp walks the loop (uniform control flow); one elected lane arms the barrier and issues the copies.
       uint32_t ring = 0;
-      int n_item = 0;
-      for (int k = item_begin; k < item_end; ++k, ++n_item) {
+      int n_item = 0; // items with at least one step (the others are skipped by every role)
+      for (int k = item_begin; k < item_end; ++k) {
         const DevItem it = p.items[k];
         const ItemView v = uniform_view_of(it);
+        const int Ts = kSparse ? uni(p.item_steps[k]) : v.T; // key-tile steps this item visits
+        if (Ts == 0) continue;
+        const uint16_t *steps = kSparse ? p.steps + uni(it.step_off) : nullptr;
         const int head = uni(it.head), q_row0 = uni(it.q_row0), pt_off = uni(it.pt_off);
         mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
+        ++n_item;
         if (elect_one()) {
           mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes);
           for (int i = 0; i < v.nq; ++i)
@@ -193,14 +202,17 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                           q_row0 + i * kTileM);
         }
         __syncwarp();
-        for (int j0 = 0; j0 < v.T; j0 += 32) { // 32 steps at a time: each lane looks up the page of one step's tile
-          const int my_j = j0 + lane;
-          int my_page = 0;
-          if (my_j < v.T) my_page = __ldg(p.page_tables + pt_off + ((v.tile_of(my_j) * kTileN) >> p.page_log2));
-          const int cnt = min(32, v.T - j0);
+        for (int j0 = 0; j0 < Ts; j0 += 32) { // 32 steps at a time: each lane looks up the pool row of one step's tile
+          const int my_jj = j0 + lane;
+          int my_row = 0;
+          if (my_jj < Ts) {
+            const int my_tile = v.tile_of(kSparse ? (int)__ldg(steps + my_jj) : my_jj);
+            const int my_page = __ldg(p.page_tables + pt_off + ((my_tile * kTileN) >> p.page_log2));
+            my_row = (my_page * H + head) * P + ((my_tile * kTileN) & (P - 1));
+          }
+          const int cnt = min(32, Ts - j0);
           for (int j = 0; j < cnt; ++j) {
-            const int page = __shfl_sync(0xffffffffu, my_page, j);
-            const int row = (page * H + head) * P + ((v.tile_of(j0 + j) * kTileN) & (P - 1));
+            const int row = __shfl_sync(0xffffffffu, my_row, j);
 #pragma unroll
             for (int kv = 0; kv < 2; ++kv) {
               const uint32_t stage = ring % kStages;
@@ -247,11 +259,18 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                  (acc || k > 0) ? 1u : 0u);
         }
       };
-      for (int k = item_begin; k < item_end; ++k, ++n_item) {
+      for (int k = item_begin; k < item_end; ++k) {
         const DevItem it = p.items[k];
         const ItemView v = uniform_view_of(it);
+        const int Ts = kSparse ? uni(p.item_steps[k]) : v.T;
+        if (Ts == 0) continue;
+        const uint16_t *steps = kSparse ? p.steps + uni(it.step_off) : nullptr;
+        // dense step index of the item's jj-th visited step (block-sparse: read one step ahead of its use)
+        auto step_at = [&](int jj) { return kSparse ? uni((int)__ldg(steps + min(jj, Ts - 1))) : jj; };
+        int j_dense = step_at(0);
         const uint32_t r0 = ring;
         mbar_wait(bar(BAR_Q_FULL), (uint32_t)(n_item & 1), 200, dbg);
+        ++n_item;
         {
           const uint32_t stage = r0 % kStages, ph = (r0 / kStages) & 1u;
           mbar_wait(bar(BAR_KV_FULL + stage), ph, 210 + stage, dbg);
@@ -262,14 +281,16 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
               mma_commit(bar(BAR_S_FULL + i));
             }
             mma_commit(bar(BAR_KV_EMPTY + stage));
-            if (v.T == 1) mma_commit(bar(BAR_Q_EMPTY));
+            if (Ts == 1) mma_commit(bar(BAR_Q_EMPTY));
           }
           __syncwarp();
         }
-        for (int j = 0; j < v.T; ++j) {
+        for (int j = 0; j < Ts; ++j) {
+          const int jd = j_dense;
+          j_dense = step_at(j + 1);
           const uint32_t rv = r0 + 2u * (uint32_t)j + 1u;
           const uint32_t stage_v = rv % kStages, ph_v = (rv / kStages) & 1u;
-          const bool has_next = (j + 1) < v.T;
+          const bool has_next = (j + 1) < Ts;
           const uint32_t rk = rv + 1u;
           const uint32_t stage_k = rk % kStages, ph_k = (rk / kStages) & 1u;
           SLACK_TRACE(2, j, 0);
@@ -277,9 +298,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           SLACK_TRACE(2, j, 1);
           {
             // masked key rows of V must be zero: P is 0 there, but 0 * NaN/Inf garbage would poison O
-            const int tile = v.tile_of(j);
-            const int c_lo = max(0, v.lo_of(j) - tile * kTileN);
-            const int c_hi = min(kTileN, v.hi_of(j) - tile * kTileN);
+            const int tile = v.tile_of(jd);
+            const int c_lo = max(0, v.lo_of(jd) - tile * kTileN);
+            const int c_hi = min(kTileN, v.hi_of(jd) - tile * kTileN);
             if (c_lo > 0 || c_hi < kTileN) {
               const int n_zero = c_lo + (kTileN - c_hi);
               const uint32_t base = sKV + stage_v * kTileBytes;
@@ -313,7 +334,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                 mma_commit(bar(BAR_S_FULL + i));
                 if (i == v.nq - 1) {
                   mma_commit(bar(BAR_KV_EMPTY + stage_k));
-                  if (j + 2 == v.T) mma_commit(bar(BAR_Q_EMPTY));
+                  if (j + 2 == Ts) mma_commit(bar(BAR_Q_EMPTY));
                 }
               } else {
                 mma_commit(bar(BAR_O_FINAL + i));
@@ -325,7 +346,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             if (!has_next) itn[i]++;
           }
         }
-        ring = r0 + 2u * (uint32_t)v.T;
+        ring = r0 + 2u * (uint32_t)Ts;
       }
     }
   } else {
@@ -344,8 +365,31 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       const DevItem it = p.items[k];
       const ItemView v = view_of(it);
       if (i >= v.nq) continue;
+      const int Ts = kSparse ? p.item_steps[k] : v.T;
+      const uint16_t *steps = kSparse ? p.steps + it.step_off : nullptr;
+      if (Ts == 0) { // block-sparse: no selected key tile in this item: out = 0, lse = -inf; no barrier is touched
+        const int local_row = i * kTileM + row;
+        if (local_row < it.q_rows) {
+          if (it.partial_slot < 0) {
+            uint4 *dst = reinterpret_cast<uint4 *>(reinterpret_cast<__nv_bfloat16 *>(p.out) +
+                                                   ((size_t)(it.q_row0 + local_row) * H + it.head) * 128);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) dst[e] = make_uint4(0u, 0u, 0u, 0u);
+            if (p.lse != nullptr) p.lse[(size_t)it.head * p.total_q + it.q_row0 + local_row] = -INFINITY;
+          } else {
+            float4 *dst = reinterpret_cast<float4 *>(p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * 128);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) dst[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+            p.ws_lse[(size_t)it.partial_slot * kItemRows + local_row] = -INFINITY;
+          }
+        }
+        continue;
+      }
       float m = -INFINITY, l = 0.f;
-      for (int j = 0; j < v.T; ++j) {
+      int j_dense = kSparse ? (int)__ldg(steps) : 0;
+      for (int j = 0; j < Ts; ++j) {
+        const int jd = j_dense; // dense step index (block-sparse: the next one is fetched a step ahead)
+        j_dense = kSparse ? (int)__ldg(steps + min(j + 1, Ts - 1)) : j + 1;
         SLACK_TRACE(i, j, 0);
         mbar_wait(bar(BAR_S_FULL + i), cnt & 1u, 300 + i, dbg);
         tc_fence_after();
@@ -360,9 +404,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         }
         tmem_wait_ld();
         SLACK_TRACE(i, j, 2);
-        const int tile = v.tile_of(j);
-        const int c_lo = max(0, v.lo_of(j) - tile * kTileN);
-        const int c_hi = min(kTileN, v.hi_of(j) - tile * kTileN);
+        const int tile = v.tile_of(jd);
+        const int c_lo = max(0, v.lo_of(jd) - tile * kTileN);
+        const int c_hi = min(kTileN, v.hi_of(jd) - tile * kTileN);
         if (c_lo > 0 || c_hi < kTileN) {
 #pragma unroll
           for (int e = 0; e < 128; ++e) s[e] = (e >= c_lo && e < c_hi) ? s[e] : -INFINITY;
@@ -539,17 +583,21 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 size_t attn_tc_smem_bytes() { return kSmemBytes; }
 
 cudaError_t attn_tc_configure() {
-  cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(attn_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(attn_tc_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
 }
 
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched) {
-  if (p.dbg_t != nullptr)
-    attn_tc_kernel<true><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+  if (p.steps != nullptr)
+    attn_tc_kernel<false, true><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+  else if (p.dbg_t != nullptr)
+    attn_tc_kernel<true, false><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
   else
-    attn_tc_kernel<false><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+    attn_tc_kernel<false, false><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
   if (n_launched) *n_launched += 1;
   return cudaGetLastError();
 }

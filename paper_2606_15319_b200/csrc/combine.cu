@@ -31,6 +31,11 @@ combine_kernel(const DevCombine *__restrict__ combines, const float *__restrict_
   constexpr size_t kSlotStride4 = (size_t)kItemRows * D / 4;
   float m = -INFINITY;
   for (int p = 0; p < cb.n_parts; ++p) m = fmaxf(m, __ldg(lse_p + (size_t)p * kItemRows));
+  if (m == -INFINITY) { // block-sparse: no part of this row had a selected key -> out = 0, lse = -inf
+    *reinterpret_cast<uint2 *>(out + ((size_t)(cb.q_row0 + r) * n_heads + cb.head) * D + lane * 4) = make_uint2(0u, 0u);
+    if (lse != nullptr && lane == 0) lse[(size_t)cb.head * total_q + cb.q_row0 + r] = -INFINITY;
+    return;
+  }
   float den = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   int p = 0;

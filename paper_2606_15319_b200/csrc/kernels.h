@@ -15,7 +15,8 @@ cudaError_t launch_kv_append(const void *k_new, const void *v_new, void *k_pool,
 // A3 (validation / fp32 path): one warp per (query row, head), fp32 accumulation, any page size.
 cudaError_t launch_attn_simt(int dtype, const void *q, const void *k_pool, const void *v_pool, void *out, float *lse,
                              const DevStream *d_streams, int n_streams, int total_q, const int32_t *d_page_tables,
-                             int n_heads, int head_dim, int page_size, float scale, cudaStream_t st, int *n_launched);
+                             int n_heads, int head_dim, int page_size, float scale, const uint32_t *mask, int mask_words,
+                             cudaStream_t st, int *n_launched);
 
 // A3 (tensor-core path, bf16, head_dim 128, page_size >= 128).
 struct TcParams {
@@ -29,6 +30,8 @@ struct TcParams {
   float *dbg_s;         // optional debug dump of the first S tiles of CTA 0 ([2][128][128] fp32), else null
   uint32_t *dbg_t;      // optional time-stamp trace [3][64][8] (selects the kTrace instantiation), else null
   unsigned long long *dbg_flag; // optional 4-word device buffer for time-out diagnostics, else null
+  const uint16_t *steps;        // block-sparse: compacted step lists (sparse_steps.cu), else null = dense
+  const int32_t *item_steps;    // block-sparse: selected steps per item
   int32_t n_heads;
   int32_t page_log2;
   int32_t total_q;
@@ -38,6 +41,10 @@ size_t attn_tc_smem_bytes();
 cudaError_t attn_tc_configure(); // cudaFuncSetAttribute(max dynamic smem); once per process/device
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched);
+
+// Block-sparse A3: per item, the selected key-tile steps under a device block mask (see sparse_steps.cu).
+cudaError_t launch_sparse_steps(const DevItem *d_items, int n_items, const uint32_t *mask, int n_heads, int mask_words,
+                                uint16_t *steps, int32_t *count, cudaStream_t st, int *n_launched);
 
 // A4: merge split-KV partials into `out` (bf16) and `lse`.
 cudaError_t launch_combine(const DevCombine *d_combines, int n_combines, const float *ws_o, const float *ws_lse, void *out,

@@ -308,6 +308,9 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     }
     DevStream d{};
     d.q_row0 = (int32_t)row;
+    d.qblock0 = out.mask_rows;
+    out.mask_rows += ceil_div(s.q_len, kItemRows);
+    out.mask_words_min = std::max<int32_t>(out.mask_words_min, ceil_div(ceil_div((int64_t)s.base + n, kTileN), 32));
     d.q_len = s.q_len;
     d.cache_len = s.cache_len;
     d.base = s.base;
@@ -414,6 +417,17 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   out.ws.o_bytes = (size_t)out.n_partial_slots * kItemRows * shape.head_dim * sizeof(float);
   out.ws.lse_off = out.ws.o_bytes;
   out.ws.total = out.ws.o_bytes + (size_t)out.n_partial_slots * kItemRows * sizeof(float);
+  // block-sparse bookkeeping: which mask row an item reads and where its compacted step list goes
+  for (DevItem &it : out.items) {
+    const DevStream &d = out.streams[it.stream];
+    it.mask_row = d.qblock0 + (it.q_row0 - d.q_row0) / kItemRows;
+    it.step_off = (int32_t)out.total_steps;
+    out.total_steps += it.sink_tiles + (it.kv_tile_end - it.kv_tile_begin);
+  }
+  if (out.total_steps > (int64_t)INT32_MAX / 2) return fail(SLACK_EINVAL, "batch too large (key-tile steps)");
+  out.sparse_steps_off = (out.ws.total + 15) & ~(size_t)15;
+  out.sparse_count_off = (out.sparse_steps_off + (size_t)out.total_steps * sizeof(uint16_t) + 15) & ~(size_t)15;
+  out.sparse_total = out.sparse_count_off + out.items.size() * sizeof(int32_t);
   return SLACK_OK;
 }
 

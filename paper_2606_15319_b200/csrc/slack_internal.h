@@ -34,7 +34,8 @@ struct DevItem {
   int32_t sink_hi;       // = base + sink (== sink_lo when the item has no sink tiles)
   int32_t sink_tile0;
   int32_t sink_tiles;
-  int32_t pad0, pad1;
+  int32_t mask_row;      // block-sparse: global 256-row query block of the item = row of the block mask (P:88 knob (2))
+  int32_t step_off;      // block-sparse: offset of the item's compacted step list (uint16 units) in the sparse workspace
 };
 static_assert(sizeof(DevItem) == 64, "DevItem layout");
 
@@ -60,7 +61,7 @@ struct DevStream {
   int32_t pt_off;
   int32_t n_table_pages;
   int32_t sink_hi;  // visible sink positions [base, sink_hi) in front of [pos_lo, pos_hi); == base when there are none
-  int32_t pad0;
+  int32_t qblock0;  // global index of the stream's first 256-row query block (row of the block mask)
 };
 static_assert(sizeof(DevStream) == 40, "DevStream layout");
 
@@ -86,6 +87,13 @@ struct HostPlan {
   std::vector<DevCombine> combines;
   int32_t n_partial_slots = 0;
   WorkspaceLayout ws;
+  // block-sparse variant (slack_chunk_attention_sparse): mask geometry and the extra workspace behind ws.total
+  int32_t mask_rows = 0;        // sum over streams of ceil(q_len / 256)
+  int32_t mask_words_min = 1;   // 32-bit words a mask row needs: ceil(max_s ceil(pos_hi / 128) / 32)
+  int64_t total_steps = 0;      // sum over items of their dense key-tile steps (entries of the step lists)
+  size_t sparse_steps_off = 0;  // byte offset of uint16 steps[total_steps] (16-byte aligned, >= ws.total)
+  size_t sparse_count_off = 0;  // byte offset of int32 item_steps[n_items]
+  size_t sparse_total = 0;      // workspace bytes slack_chunk_attention_sparse needs
   double makespan = 0, ideal = 0;    // in cost units (for tests / tuning)
 };
 

@@ -193,3 +193,19 @@ def test_empty_batches_are_legal(hctx):
     empty = [W.StreamSpec(0, s.cache_len, s.base, s.window, 0, s.page_table) for s in w.streams]
     plan = hctx.slack_plan(_pool(w), empty)
     assert plan.num_items == 0
+
+
+def test_sparse_plan_geometry(hctx):
+    """Mask geometry and workspace the block-sparse call needs (include/slack.h): rows = sum ceil(Lq/256); words cover the
+    last key block of the longest stream; the sparse workspace holds the split-KV partials plus one uint16 per dense
+    key-tile step and one int32 per item."""
+    w = W.small_ragged(page_size=256)
+    pool = binding.Pool(None, None, w.n_pages, w.n_heads, w.head_dim, w.page_size, w.dtype)
+    plan = hctx.slack_plan(pool, w.streams, force_splits=2)
+    assert plan.mask_rows == sum(-(-s.q_len // 256) for s in w.streams)
+    assert plan.mask_min_words == -(-max(-(-(s.base + s.n) // 128) for s in w.streams) // 32)
+    items = plan.items()
+    steps = sum(it["sink_tiles"] + it["kv_tile_end"] - it["kv_tile_begin"] for it in items)
+    assert plan.sparse_workspace_bytes >= plan.workspace_bytes + 2 * steps + 4 * len(items)
+    packed = W.pack_block_masks(w, W.random_block_masks(w, 0.5, seed=1))
+    assert packed.shape == (plan.mask_rows, w.n_heads, plan.mask_min_words)
