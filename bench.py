@@ -7,6 +7,8 @@ Every layer has its own pools and its own seeded Q / K_new / V_new, so each laun
 (cfg2: 201 MB of pools per layer, 6 GB per step >> 126 MB L2) — no explicit L2 flush is needed.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg4|cfg5|cfg5b] [--impl reference]
+                    [--sparsity RHO]   block-sparse variant (P:88 knob (2), rho in {.6,.7,.8,.9} P:568): every layer gets
+                                       its own seeded block mask; flops count the SELECTED (query, key) pairs only
 
 value   = attention FLOPs (4*H*D*sum Lq*Lk, visible keys only) of all ranks / device time of the K steps (max over ranks)
 e2e     = the same with Q/K_new/V_new copied from pinned host memory and Out copied back inside the timed region
@@ -47,6 +49,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=768, help="query rows of the oracle sample")
+    ap.add_argument("--sparsity", type=float, default=0.0, help="block-sparse variant: fraction of visible key blocks dropped")
     return ap.parse_args()
 
 
@@ -148,14 +151,35 @@ def sample_flops(streams, rows, n_heads, head_dim):
     return 4.0 * n_heads * head_dim * sum(len(r) * lk for r, lk in zip(rows, metrics.visible_keys(streams)))
 
 
-def time_oracle(w, k_pool, v_pool, q, n_rows):
+def selected_pairs(w, masks, rows=None):
+    """(query, key) pairs, summed over heads, that a block mask leaves: sum over query rows of the visible keys in selected
+    blocks.  `rows`: optional per-stream sampled rows (else every row)."""
+    from paper_2606_15319_b200 import workloads as W
+    total = 0
+    for si, (s, m) in enumerate(zip(w.streams, masks)):
+        if s.q_len == 0:
+            continue
+        n = s.cache_len + s.q_len
+        lo = max(0, n - s.window) if s.window > 0 else 0
+        sink = min(s.sink_len, n)
+        lo = max(lo, sink)
+        toks = np.concatenate([np.arange(0, sink), np.arange(lo, n)])
+        keys_per_block = np.bincount((s.base + toks) // W.MASK_BLOCK_K, minlength=m.shape[2])
+        per_qb = (m * keys_per_block[None, None, :]).sum(axis=(0, 2))           # [n_qb], summed over heads
+        r = np.arange(s.q_len) if rows is None else np.asarray(rows[si])
+        total += int(per_qb[r // W.MASK_BLOCK_Q].sum())
+    return total
+
+
+def time_oracle(w, k_pool, v_pool, q, n_rows, masks=None):
     """Runs oracle.chunk_attention on `n_rows` sampled rows; returns (seconds, flops, rows, out, lse)."""
     import oracle
     rows = sample_rows(w.streams, n_rows)
     t0 = time.perf_counter()
-    out, lse = oracle.chunk_attention(k_pool, v_pool, w.streams, q, w.scale, w.dtype, rows=rows)
+    out, lse = oracle.chunk_attention(k_pool, v_pool, w.streams, q, w.scale, w.dtype, rows=rows, block_masks=masks)
     dt = time.perf_counter() - t0
-    return dt, sample_flops(w.streams, rows, w.n_heads, w.head_dim), rows, out, lse
+    fl = sample_flops(w.streams, rows, w.n_heads, w.head_dim) if masks is None else 4.0 * w.head_dim * selected_pairs(w, masks, rows)
+    return dt, fl, rows, out, lse
 
 
 def host_layer(w, seed):
@@ -174,15 +198,19 @@ def run_reference(args):
         return
     w = make_descriptors(args)
     k_pool, v_pool, q = host_layer(w, seed=12345)
+    masks = None
+    if args.sparsity > 0:
+        from paper_2606_15319_b200 import workloads as W
+        masks = W.random_block_masks(w, args.sparsity, seed=9000)
     # size the per-step sample so that warmup+steps finish within a few minutes (about 4 s of CPU per step)
-    time_oracle(w, k_pool, v_pool, q, 64)                                   # cold pass (imports, page faults)
-    dt, fl, *_ = time_oracle(w, k_pool, v_pool, q, 64)
+    time_oracle(w, k_pool, v_pool, q, 64, masks)                                   # cold pass (imports, page faults)
+    dt, fl, *_ = time_oracle(w, k_pool, v_pool, q, 64, masks)
     n_rows = int(max(64, min(w.total_q, 64 * 4.0 / max(dt, 1e-3))))
     for _ in range(args.warmup):
-        time_oracle(w, k_pool, v_pool, q, n_rows)
+        time_oracle(w, k_pool, v_pool, q, n_rows, masks)
     t, f = 0.0, 0.0
     for _ in range(args.steps):
-        dt, fl, *_ = time_oracle(w, k_pool, v_pool, q, n_rows)
+        dt, fl, *_ = time_oracle(w, k_pool, v_pool, q, n_rows, masks)
         t += dt
         f += fl
     val = f / t / 1e12
@@ -192,7 +220,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_label(args, w), "sample": sample},
+        "config": {"workload": workload_label(args, w), "sample": sample, "sparsity": args.sparsity},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -242,7 +270,14 @@ def run_ours(args):
         outs.append(torch.empty(tq, H, D, device=dev, dtype=torch.bfloat16))
     main = torch.cuda.current_stream()
     plan0 = ctx.slack_plan(pools[0], w.streams, force_splits=args.force_splits)
-    ws = torch.empty(max(plan0.workspace_bytes, 256), dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(plan0.workspace_bytes, plan0.sparse_workspace_bytes if args.sparsity > 0 else 0, 256),
+                     dtype=torch.uint8, device=dev)
+    # block-sparse variant: a seeded mask per layer (the selection rule, Light Forcing's [39] P:319, is outside the path)
+    layer_masks, masks_d = None, None
+    if args.sparsity > 0:
+        from paper_2606_15319_b200 import workloads as W
+        layer_masks = [W.random_block_masks(w, args.sparsity, seed=9000 + 100 * rank + l) for l in range(L)]
+        masks_d = [torch.from_numpy(W.pack_block_masks(w, m).view(np.int32)).to(dev) for m in layer_masks]
     plan_info = {"items": plan0.num_items, "partial_slots": plan0.num_partial_slots, "kernel_kind": plan0.kernel_kind}
     keep_plans = [plan0]
     state = {"launches": 0, "plan_s": 0.0}
@@ -257,7 +292,11 @@ def run_ours(args):
             pre(l)
             ctx.slack_kv_append_planned(plan, pools[l], kn_of(l), vn_of(l), stream=main)             # A1
             state["launches"] += ctx.last_launch_count
-            ctx.slack_chunk_attention(plan, pools[l], q_of(l), out_of(l), w.scale, workspace=ws, stream=main)  # A3 + A4
+            if masks_d is None:
+                ctx.slack_chunk_attention(plan, pools[l], q_of(l), out_of(l), w.scale, workspace=ws, stream=main)  # A3 + A4
+            else:
+                ctx.slack_chunk_attention_sparse(plan, pools[l], q_of(l), out_of(l), w.scale, masks_d[l], workspace=ws,
+                                                 stream=main)
             state["launches"] += ctx.last_launch_count
             post(l)
 
@@ -287,8 +326,13 @@ def run_ours(args):
             ms = float(t.item())
         return ms
 
-    flops_layer = metrics.attention_flops(w.streams, H, D)
-    flops_step = flops_layer * L
+    if layer_masks is None:
+        flops_layer = metrics.attention_flops(w.streams, H, D)
+        flops_step = flops_layer * L
+    else:                                             # selected (query, key) pairs only
+        per_layer = [4.0 * D * selected_pairs(w, m) for m in layer_masks]
+        flops_step = float(sum(per_layer))
+        flops_layer = flops_step / L
 
     # ---- device-resident timing (value) + per-kernel roofline ------------------------------------------------------
     sampler = ClockSampler(local) if rank == 0 else None
@@ -372,13 +416,28 @@ def run_ours(args):
         peak, which = 1400.0, "fallback: B200_PROFILING.md sustained ~1.4 PFLOP/s (MEASURED_PEAKS.json absent)"
     kernel_ms = k_ms / max(k_n, 1)
     achieved = flops_layer / (kernel_ms * 1e-3) / 1e12 if k_n else None
-    roofline = {"bound": "tensor", "kernel": "attn_tc_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-                "peak_source": which, "kernel_ms_avg": kernel_ms, "launches_timed": k_n,
-                "flops_per_launch": flops_layer,
-                "frac_of_burst": (achieved / float(peaks["bf16_tflops"])) if achieved and "bf16_tflops" in peaks else None,
-                "frac_of_nominal_2250": (achieved / 2250.0) if achieved else None,
-                "kernel_share_of_step": (k_ms / ms) if k_n else None}
+    # minimal HBM bytes of one launch: Q read, Out written, every visible K and V read once per (stream, head)
+    bytes_layer = float(sum(H * (2 * s.q_len + 2 * lk) * D * 2 for s, lk in zip(w.streams, metrics.visible_keys(w.streams))))
+    hbm_peak = float(peaks.get("hbm_gbs", 6500.0))
+    intensity = flops_layer / bytes_layer
+    if layer_masks is None and intensity < peak * 1e12 / (hbm_peak * 1e9):
+        # decode-like short chunks (cfg5b): fewer flops per K/V byte than the ridge point -> HBM-bound
+        gbs = bytes_layer / (kernel_ms * 1e-3) / 1e9 if k_n else None
+        roofline = {"bound": "hbm", "kernel": "attn_tc_kernel", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": (gbs / hbm_peak) if gbs else None, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                    "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6500 GB/s",
+                    "kernel_ms_avg": kernel_ms, "launches_timed": k_n, "bytes_per_launch": bytes_layer,
+                    "flops_per_byte": intensity, "ridge_flops_per_byte": peak * 1e12 / (hbm_peak * 1e9),
+                    "tflops": achieved, "kernel_share_of_step": (k_ms / ms) if k_n else None}
+    else:
+        roofline = {"bound": "tensor", "kernel": "attn_tc_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                    "frac": (achieved / peak) if achieved else None,
+                    "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if layer_masks is None else None,
+                    "peak_source": which, "kernel_ms_avg": kernel_ms, "launches_timed": k_n,
+                    "flops_per_launch": flops_layer,
+                    "frac_of_burst": (achieved / float(peaks["bf16_tflops"])) if achieved and "bf16_tflops" in peaks else None,
+                    "frac_of_nominal_2250": (achieved / 2250.0) if achieved else None,
+                    "kernel_share_of_step": (k_ms / ms) if k_n else None}
 
     # ---- CPU baseline: the oracle on layer 0 of this very run (also a live parity spot check) ----------------------
     cpu = None
@@ -387,10 +446,11 @@ def run_ours(args):
         kp0 = binding.to_numpy(pools[0].k_pool, "bf16")
         vp0 = binding.to_numpy(pools[0].v_pool, "bf16")
         q0 = binding.to_numpy(qs[0], "bf16")
-        time_oracle(w, kp0, vp0, q0, 64)                                    # cold pass (imports, page faults)
-        dt, fl, rows, o_want, _ = time_oracle(w, kp0, vp0, q0, 64)          # calibration pass
+        m0 = layer_masks[0] if layer_masks is not None else None
+        time_oracle(w, kp0, vp0, q0, 64, m0)                                # cold pass (imports, page faults)
+        dt, fl, rows, o_want, _ = time_oracle(w, kp0, vp0, q0, 64, m0)      # calibration pass
         n_rows = int(max(64, min(tq, 64 * 15.0 / max(dt, 1e-3), args.cpu_rows * 64)))
-        dt, fl, rows, o_want, _ = time_oracle(w, kp0, vp0, q0, n_rows)
+        dt, fl, rows, o_want, _ = time_oracle(w, kp0, vp0, q0, n_rows, m0)
         import oracle
         ma, rf = oracle.error_metrics(outs[0].float().cpu().numpy().astype(np.float64), o_want)
         parity = {"rows": int(sum(len(r) for r in rows)), "max_abs": ma, "rel_fro": rf, "pass": bool(ma <= 2e-2 and rf <= 1e-2)}
@@ -405,7 +465,9 @@ def run_ours(args):
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "plan": plan_info,
                        "flops_per_step": flops_step, "chunk_layers_per_s": world * len(w.streams) * L * args.steps / (ms * 1e-3),
                        "chunks_per_s_30_layers_1_step": world * len(w.streams) * args.steps / (ms * 1e-3) * (L / 30.0),
-                       "plan_ms_per_step_host": plan_ms},
+                       "plan_ms_per_step_host": plan_ms,
+                       "sparsity": args.sparsity if layer_masks is not None else 0.0,
+                       "dense_flops_per_step": metrics.attention_flops(w.streams, H, D) * L},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "parity_spot_check": parity}
     print(json.dumps(line))
