@@ -33,6 +33,11 @@ rule from Light Forcing [39] P:319 - the rule is NOT in the paper, so the mask i
     t is used iff it is visible (above) AND mask[h, qb, kb]
     out_i = softmax over the used keys; a row with no used key has out_i = 0 and lse_i = -inf.
 
+State-plane page transfer ("transfer(stream, src, dst, page_range)"
+layer-major asynchronous streaming, "migrates only the KV pages corresponding to the head partition"):
+an exact copy, for every layer, of the head slices [h0, h1) of the listed source pages into the listed destination
+pages of another pool; nothing else in the destination changes (`kv_transfer`).
+
 Since attention is a *defined* function the oracle is that definition written out: gather, one
 matmul, a max-subtracted exp, one matmul, a division - in fp64, no tiling over keys, no online
 softmax, no splits.  Query rows are processed in blocks of <= `row_block` rows only to bound
@@ -114,6 +119,21 @@ def gather_kv(pool: np.ndarray, stream, tokens: np.ndarray) -> np.ndarray:
     """Rows of one pool for the given logical tokens of one stream -> [len(tokens), H, D] (storage dtype)."""
     page, slot = token_slots(stream, tokens, pool.shape[2])
     return pool[page, :, slot, :]
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4: state-plane page transfer (exact copy, P:255, P:660-662)
+# ----------------------------------------------------------------------------------------------
+
+def kv_transfer(src_k: np.ndarray, src_v: np.ndarray, dst_k: np.ndarray, dst_v: np.ndarray,
+                src_pages: Sequence[int], dst_pages: Sequence[int], head_begin: int, head_end: int) -> None:
+    """One layer of transfer(stream, src, dst, page_range): page src_pages[i] of the source pool image becomes page
+    dst_pages[i] of the destination pool image, heads [head_begin, head_end) only (the head partition of P:660-662);
+    in place on dst_*; pools are [n_pages, H, P, D] of the same H, P, D and storage dtype."""
+    assert len(src_pages) == len(dst_pages)
+    for sp, dp in zip(src_pages, dst_pages):
+        dst_k[dp, head_begin:head_end] = src_k[sp, head_begin:head_end]
+        dst_v[dp, head_begin:head_end] = src_v[sp, head_begin:head_end]
 
 
 # ----------------------------------------------------------------------------------------------
