@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-rows", type=int, default=768, help="query rows of the oracle sample")
+    ap.add_argument("--transfer-bench", action="store_true",
+                    help="also time slack_kv_transfer (state-plane page transfer, NEXT-4) of stream 0 over all layers")
     ap.add_argument("--sparsity", type=float, default=0.0, help="block-sparse variant: fraction of visible key blocks dropped")
     return ap.parse_args()
 
@@ -397,6 +399,37 @@ def run_ours(args):
         torch.cuda.synchronize()
         assert torch.equal(hout[L - 1], outs[L - 1].cpu()), "e2e output differs from the device-resident run"
 
+    # ---- state-plane page transfer (NEXT-4): stream 0's pages, all layers, HBM pool -> second HBM pool ----------------
+    xfer = None
+    if args.transfer_bench and rank == 0:
+        s0 = w.streams[0]
+        sp = np.asarray(s0.page_table, dtype=np.int32)
+        dst_pools = []
+        for l in range(L):
+            kp = torch.empty(sp.size, H, P, D, device=dev, dtype=torch.bfloat16)
+            dst_pools.append(binding.Pool(kp, torch.empty_like(kp), int(sp.size), H, D, P, "bf16"))
+        dp = np.random.default_rng(3).permutation(sp.size).astype(np.int32)
+        for _ in range(3):
+            ctx.slack_kv_transfer(pools, dst_pools, sp, dp, 0, H, stream=main)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 5
+        e0.record(main)
+        for _ in range(reps):
+            ctx.slack_kv_transfer(pools, dst_pools, sp, dp, 0, H, stream=main)
+        e1.record(main)
+        torch.cuda.synchronize()
+        x_ms = e0.elapsed_time(e1) / reps
+        x_bytes = 2.0 * 2.0 * sp.size * H * P * D * 2 * L          # K and V, read + write, all layers
+        same = all(torch.equal(dst_pools[l].k_pool[int(dp[i])], pools[l].k_pool[int(sp[i])]) for l in (0, L - 1) for i in (0, sp.size - 1))
+        xfer = {"pages": int(sp.size), "layers": L, "bytes_moved": x_bytes, "ms": x_ms, "GB_per_s": x_bytes / (x_ms * 1e-3) / 1e9,
+                "frac_of_hbm_peak": None, "spot_check_equal": bool(same), "kernel": "kv_transfer_kernel, one launch per layer"}
+        try:
+            xfer["frac_of_hbm_peak"] = xfer["GB_per_s"] / float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+        except Exception:
+            pass
+        del dst_pools
+
     if dist is not None:
         dist.barrier()
     if rank != 0:
@@ -470,6 +503,8 @@ def run_ours(args):
                        "dense_flops_per_step": metrics.attention_flops(w.streams, H, D) * L},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "parity_spot_check": parity}
+    if xfer is not None:
+        line["transfer"] = xfer
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

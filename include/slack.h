@@ -175,6 +175,27 @@ size_t slack_plan_sparse_workspace_bytes(const slack_plan_t *plan);
 int32_t slack_plan_mask_rows(const slack_plan_t *plan);      /* sum over streams of ceil(q_len / 256)                 */
 int32_t slack_plan_mask_min_words(const slack_plan_t *plan); /* ceil(max over streams of ceil((base+Lc+Lq)/128) / 32) */
 
+/* ---- state-plane page transfer -------------------------------------------------------------- */
+/* PAPER.md P:255 "transfer(stream, src, dst, page_range)": the single primitive behind credit-aware eviction,
+ * re-homing and elastic SP; requests return immediately, run on a dedicated CUDA stream,
+ * and are issued in LAYER-MAJOR order so the destination can start layer k once layer k's pages have arrived;
+ * only the head partition assigned to the donor worker moves.
+ * For each layer l = 0 .. n_layers-1, in order: page src_page_ids[i] of src_pools[l] is copied, bit for bit, into page
+ * dst_page_ids[i] of dst_pools[l], heads [head_begin, head_end) only (in the [n_pages][H][P][D] layout a page's head
+ * slice is one contiguous run); no other byte of the destination changes.  One kernel per layer on `cuda_stream`
+ * (asynchronous: give it a side stream to overlap with compute); if layer_done_events is not NULL, entry l (a
+ * cudaEvent_t, may be NULL) is recorded right after layer l's copy, which is what a consumer of layer l waits for.
+ * src_pools / dst_pools: HOST arrays of n_layers descriptors; all layers of one side share n_pages, both sides share
+ * n_heads, head_dim, page_size and dtype; the pool pointers are unified virtual addresses valid on this device: HBM of
+ * this GPU, pinned (mapped) host memory for eviction / offload, or a peer GPU's HBM with peer access enabled.
+ * src_page_ids / dst_page_ids: HOST int32[n_pages], read during the call; destination ids must be distinct.  The
+ * caller's page tables are its own business: after the transfer the stream's table on the destination side is
+ * dst_page_ids in the same logical order.  Errors: SLACK_EINVAL for ids out of range, duplicate destinations, mismatched
+ * shapes or an empty head range. */
+slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_pool *src_pools, const slack_pool *dst_pools,
+                               int32_t n_pages, const int32_t *src_page_ids, const int32_t *dst_page_ids,
+                               int32_t head_begin, int32_t head_end, void *cuda_stream, void *const *layer_done_events);
+
 /* Number of kernels the last slack_chunk_attention / slack_kv_append call on this ctx launched (bench bookkeeping). */
 int32_t slack_last_launch_count(const slack_ctx *ctx);
 

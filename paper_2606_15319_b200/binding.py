@@ -69,6 +69,8 @@ SYMBOLS = {
     "slack_plan_sparse_workspace_bytes": (C.c_size_t, [_VP]),
     "slack_plan_mask_rows": (C.c_int32, [_VP]),
     "slack_plan_mask_min_words": (C.c_int32, [_VP]),
+    "slack_kv_transfer": (C.c_int, [_VP, C.c_int32, C.POINTER(CPool), C.POINTER(CPool), C.c_int32, C.POINTER(C.c_int32),
+                                   C.POINTER(C.c_int32), C.c_int32, C.c_int32, _VP, C.POINTER(_VP)]),
     "slack_profile_attention": (C.c_int, [_VP, C.c_int32]),
     "slack_profile_read": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_int32)]),
     "slack_debug_set": (C.c_int, [_VP, C.c_int32, _VP]),
@@ -252,6 +254,24 @@ class Context:
                                                           _ptr(lse), C.c_float(scale), _ptr(block_mask),
                                                           int(block_mask.shape[-1]), _ptr(workspace), ws_bytes,
                                                           _cuda_stream(stream)))
+
+    def slack_kv_transfer(self, src_pools: Sequence[Pool], dst_pools: Sequence[Pool], src_page_ids, dst_page_ids,
+                          head_begin: int, head_end: int, stream=None, layer_done_events=None) -> None:
+        """Layer-major page transfer (include/slack.h).  layer_done_events: optional list of torch.cuda.Event (one per
+        layer, already created with .record()-able handles) recorded after each layer's copy."""
+        n_layers = len(src_pools)
+        assert len(dst_pools) == n_layers
+        sp = (CPool * max(n_layers, 1))(*[p.c for p in src_pools])
+        dp = (CPool * max(n_layers, 1))(*[p.c for p in dst_pools])
+        a = np.ascontiguousarray(src_page_ids, dtype=np.int32)
+        b = np.ascontiguousarray(dst_page_ids, dtype=np.int32)
+        assert a.size == b.size
+        ev = None
+        if layer_done_events is not None:
+            ev = (_VP * n_layers)(*[int(e.cuda_event) for e in layer_done_events])
+        self._check(self.lib.slack_kv_transfer(self.handle, n_layers, sp, dp, int(a.size),
+                                               a.ctypes.data_as(C.POINTER(C.c_int32)), b.ctypes.data_as(C.POINTER(C.c_int32)),
+                                               int(head_begin), int(head_end), _cuda_stream(stream), ev))
 
     # --- measurement ---------------------------------------------------------------------------------------------------
     def profile_attention(self, enable: bool) -> None:

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <new>
 #include <string>
@@ -31,6 +32,12 @@ struct slack_ctx {
   size_t stage_cap = 0;
   cudaEvent_t stage_ev = nullptr;
   bool stage_pending = false;
+  // staging for slack_kv_transfer (source / destination page id lists)
+  void *h_xfer = nullptr;
+  void *d_xfer = nullptr;
+  size_t xfer_cap = 0;
+  cudaEvent_t xfer_ev = nullptr;
+  bool xfer_pending = false;
   // plan tables are uploaded on a private non-blocking stream: slack_plan never waits for the caller's queued work
   cudaStream_t up_stream = nullptr;
   // diagnostics
@@ -162,6 +169,10 @@ void slack_destroy(slack_ctx *ctx) {
     if (ctx->up_stream) cudaStreamDestroy(ctx->up_stream);
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
     if (ctx->d_stage) cudaFree(ctx->d_stage);
+    if (ctx->xfer_pending) cudaEventSynchronize(ctx->xfer_ev);
+    if (ctx->xfer_ev) cudaEventDestroy(ctx->xfer_ev);
+    if (ctx->h_xfer) cudaFreeHost(ctx->h_xfer);
+    if (ctx->d_xfer) cudaFree(ctx->d_xfer);
     if (ctx->h_dbg) cudaFreeHost(ctx->h_dbg);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
   }
@@ -396,6 +407,79 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
   SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, reinterpret_cast<DevStream *>(d), hp.n_streams,
                                    max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.head_dim, hp.page_size,
                                    elem_bytes(hp.dtype), ctx->sm_count, cs, &ctx->last_launches));
+  return SLACK_OK;
+}
+
+/* ------------------------------------------------------------------------------------------------ state-plane transfer */
+slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_pool *src_pools, const slack_pool *dst_pools,
+                               int32_t n_pages, const int32_t *src_page_ids, const int32_t *dst_page_ids,
+                               int32_t head_begin, int32_t head_end, void *cuda_stream, void *const *layer_done_events) {
+  if (!ctx) return SLACK_EINVAL;
+  ctx->last_launches = 0;
+  slack_status st = ensure_device(ctx);
+  if (st != SLACK_OK) return st;
+  if (n_layers < 0 || n_pages < 0) return set_err(ctx, SLACK_EINVAL, "negative n_layers / n_pages");
+  if (n_layers == 0 || n_pages == 0) return SLACK_OK;
+  if (!src_pools || !dst_pools || !src_page_ids || !dst_page_ids) return set_err(ctx, SLACK_EINVAL, "NULL argument");
+  const slack_pool &s0 = src_pools[0];
+  const slack_pool &d0 = dst_pools[0];
+  if (s0.n_heads <= 0 || s0.head_dim <= 0 || s0.page_size <= 0 || (s0.dtype != SLACK_BF16 && s0.dtype != SLACK_F32))
+    return set_err(ctx, SLACK_EINVAL, "bad source pool shape / dtype");
+  if (((size_t)s0.page_size * s0.head_dim * elem_bytes(s0.dtype)) % 16 != 0)
+    return set_err(ctx, SLACK_EUNSUPPORTED, "a (page, head) slice must be a multiple of 16 bytes");
+  if (head_begin < 0 || head_end > s0.n_heads || head_begin >= head_end)
+    return set_err(ctx, SLACK_EINVAL, "head range must satisfy 0 <= head_begin < head_end <= n_heads");
+  for (int32_t l = 0; l < n_layers; ++l) {
+    const slack_pool &a = src_pools[l];
+    const slack_pool &b = dst_pools[l];
+    if ((st = check_pool(ctx, &a, nullptr)) != SLACK_OK || (st = check_pool(ctx, &b, nullptr)) != SLACK_OK) return st;
+    if (a.n_heads != s0.n_heads || a.head_dim != s0.head_dim || a.page_size != s0.page_size || a.dtype != s0.dtype ||
+        a.n_pages != s0.n_pages || b.n_heads != s0.n_heads || b.head_dim != s0.head_dim || b.page_size != s0.page_size ||
+        b.dtype != s0.dtype || b.n_pages != d0.n_pages)
+      return set_err(ctx, SLACK_EINVAL, "all layers' pools must share one shape per side, and both sides H, D, P and dtype");
+  }
+  {
+    std::vector<uint8_t> seen((size_t)std::max(d0.n_pages, 0), 0);
+    for (int32_t i = 0; i < n_pages; ++i) {
+      if (src_page_ids[i] < 0 || src_page_ids[i] >= s0.n_pages) return set_err(ctx, SLACK_EINVAL, "source page id out of range");
+      if (dst_page_ids[i] < 0 || dst_page_ids[i] >= d0.n_pages) return set_err(ctx, SLACK_EINVAL, "destination page id out of range");
+      if (seen[dst_page_ids[i]]) return set_err(ctx, SLACK_EINVAL, "destination page listed twice");
+      seen[dst_page_ids[i]] = 1;
+    }
+  }
+  cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const size_t half = align_up((size_t)n_pages * sizeof(int32_t), 256);
+  const size_t total = 2 * half;
+  if (ctx->xfer_pending) { // the previous transfer's upload must have consumed the staging buffer
+    SLACK_CUDA(ctx, cudaEventSynchronize(ctx->xfer_ev));
+    ctx->xfer_pending = false;
+  }
+  if (!ctx->xfer_ev) SLACK_CUDA(ctx, cudaEventCreateWithFlags(&ctx->xfer_ev, cudaEventDisableTiming));
+  if (total > ctx->xfer_cap) {
+    if (ctx->h_xfer) cudaFreeHost(ctx->h_xfer);
+    if (ctx->d_xfer) cudaFree(ctx->d_xfer); // device-synchronising: earlier transfers have finished with it
+    ctx->h_xfer = ctx->d_xfer = nullptr;
+    ctx->xfer_cap = 0;
+    const size_t cap = align_up(total * 2, 4096);
+    SLACK_CUDA(ctx, cudaMallocHost(&ctx->h_xfer, cap));
+    SLACK_CUDA(ctx, cudaMalloc(&ctx->d_xfer, cap));
+    ctx->xfer_cap = cap;
+  }
+  uint8_t *h = reinterpret_cast<uint8_t *>(ctx->h_xfer);
+  memcpy(h, src_page_ids, (size_t)n_pages * sizeof(int32_t));
+  memcpy(h + half, dst_page_ids, (size_t)n_pages * sizeof(int32_t));
+  SLACK_CUDA(ctx, cudaMemcpyAsync(ctx->d_xfer, h, total, cudaMemcpyHostToDevice, cs));
+  SLACK_CUDA(ctx, cudaEventRecord(ctx->xfer_ev, cs));
+  ctx->xfer_pending = true;
+  const int32_t *d_src = reinterpret_cast<const int32_t *>(ctx->d_xfer);
+  const int32_t *d_dst = reinterpret_cast<const int32_t *>(reinterpret_cast<uint8_t *>(ctx->d_xfer) + half);
+  for (int32_t l = 0; l < n_layers; ++l) { // layer-major: layer l is complete when event l fires
+    SLACK_CUDA(ctx, launch_kv_transfer(src_pools[l].k_pool, src_pools[l].v_pool, dst_pools[l].k_pool, dst_pools[l].v_pool,
+                                       d_src, d_dst, n_pages, s0.n_heads, s0.head_dim, s0.page_size, elem_bytes(s0.dtype),
+                                       head_begin, head_end, ctx->sm_count, cs, &ctx->last_launches));
+    if (layer_done_events && layer_done_events[l])
+      SLACK_CUDA(ctx, cudaEventRecord(reinterpret_cast<cudaEvent_t>(layer_done_events[l]), cs));
+  }
   return SLACK_OK;
 }
 

@@ -46,6 +46,12 @@ cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUt
 cudaError_t launch_sparse_steps(const DevItem *d_items, int n_items, const uint32_t *mask, int n_heads, int mask_words,
                                 uint16_t *steps, int32_t *count, cudaStream_t st, int *n_launched);
 
+// NEXT-4: one layer of the state-plane page transfer (see transfer.cu).
+cudaError_t launch_kv_transfer(const void *src_k, const void *src_v, void *dst_k, void *dst_v, const int32_t *d_src_ids,
+                               const int32_t *d_dst_ids, int n_pages, int n_heads, int head_dim, int page_size,
+                               int elem_bytes, int head_begin, int head_end, int sm_count, cudaStream_t st,
+                               int *n_launched);
+
 // A4: merge split-KV partials into `out` (bf16) and `lse`.
 cudaError_t launch_combine(const DevCombine *d_combines, int n_combines, const float *ws_o, const float *ws_lse, void *out,
                            float *lse, int n_heads, int head_dim, int total_q, cudaStream_t st, int *n_launched);
