@@ -166,6 +166,32 @@ def test_late_large_logits_force_rescale(ctx):
     run_case(ctx, w, force_splits=3)
 
 
+def test_huge_logit_jumps_inside_a_tile(ctx):
+    """Keys whose logit exceeds everything seen before by 100-300 nats (>> 64 in log2 units), sitting in the first and
+    in the second 64 columns of late key tiles, once and twice on the same query row, rising and falling: the lazy-rescale
+    logic must take its exact path (true maximum, rescale, recompute) instead of overflowing.  The oracle is fp64."""
+    w = W.make_workload("huge_jumps", dtype="bf16", n_heads=2, head_dim=128, page_size=128, q_lens=[260], cache_lens=[1500],
+                        windows=[0], bases=[3], seed=35, amp=0.5)
+    q = W.bf16_bits_to_f32(w.q)
+    unit = q / np.maximum(np.linalg.norm(q, axis=-1, keepdims=True), 1e-6)         # [260, H, D]
+    kn = W.bf16_bits_to_f32(w.k_new)
+    kp = W.bf16_bits_to_f32(w.k_prior[0])
+    # own-chunk token j sits at position 3 + 1500 + j: column (1503 + j) % 128 of its tile
+    cols = {j: (1503 + j) % 128 for j in (40, 100, 200, 230, 259)}
+    assert cols[40] < 64 and cols[200] < 64 and cols[100] >= 64 and cols[259] >= 64
+    kn[40] = 250.0 * unit[40]          # first half of a tile, row 40
+    kn[100] = 300.0 * unit[100]        # second half, row 100
+    kn[200] = 200.0 * unit[7]          # row 7: first jump ...
+    kn[259] = 420.0 * unit[7]          # ... and a larger one later, second half
+    kn[230] = 150.0 * unit[40]         # row 40 again, smaller than its first jump (must not disturb it)
+    kp[700] = 180.0 * unit[100]        # an early big key for row 100 (mid-cache), overtaken later by kn[100]
+    w.k_new = W.f32_to_bf16_bits(kn)
+    w.k_prior = [W.f32_to_bf16_bits(kp)]
+    for splits in (1, 3):
+        res, out, lse, _ = run_case(ctx, w, force_splits=splits)
+        assert np.isfinite(lse).all()
+
+
 def test_all_equal_logits_and_zero_q(ctx):
     w = W.small_ragged(seed=34)
     w.q = np.zeros_like(w.q)
