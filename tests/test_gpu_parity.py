@@ -203,3 +203,18 @@ def test_all_equal_logits_and_zero_q(ctx):
             lk = len(oracle.visible_tokens(s))
             assert np.allclose(lse[:, r:r + s.q_len], np.log(lk), atol=1e-4)
         r += s.q_len
+
+
+# ------------------------------------------------------------------------------------------------ unusual shapes / sizes
+@pytest.mark.parametrize("n_heads,page_size,lq,lc,window,base", [
+    (5, 1024, 300, 70000, 0, 1023),        # long cache (550 key tiles), odd head count, base at the last slot of a page
+    (1, 128, 257, 40000, 33000, 127),      # one head, window cutting mid-tile far into the cache
+    (40, 256, 129, 515, 0, 0),             # many heads, short cache
+])
+def test_unusual_shapes_sampled_rows(ctx, n_heads, page_size, lq, lc, window, base):
+    w = W.make_workload("odd_shape", dtype="bf16", n_heads=n_heads, head_dim=128, page_size=page_size, q_lens=[lq],
+                        cache_lens=[lc], windows=[window], bases=[base], seed=77, amp=0.5, spare_pages=2)
+    rows = [np.unique(np.concatenate([[0, 127, 128, lq - 1], np.random.default_rng(5).integers(0, lq, size=24)]))]
+    for splits in (0, 1):
+        res, out, *_ = run_case(ctx, w, rows=rows, force_splits=splits)
+        assert res["kind"] == 0
