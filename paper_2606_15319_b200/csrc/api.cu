@@ -506,6 +506,8 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   if (block_mask) {
     if (!aligned(block_mask, 4)) return set_err(ctx, SLACK_EINVAL, "block_mask must be 4-byte aligned");
     if (mask_words < hp.mask_words_min) return set_err(ctx, SLACK_EINVAL, "mask_words smaller than slack_plan_mask_min_words()");
+    if (hp.max_item_steps > 65535)
+      return set_err(ctx, SLACK_EUNSUPPORTED, "block-sparse path: an item spans more than 65535 key tiles (8.3 M keys)");
   }
 
   if (hp.kernel_kind == 1) {

@@ -422,7 +422,9 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     const DevStream &d = out.streams[it.stream];
     it.mask_row = d.qblock0 + (it.q_row0 - d.q_row0) / kItemRows;
     it.step_off = (int32_t)out.total_steps;
-    out.total_steps += it.sink_tiles + (it.kv_tile_end - it.kv_tile_begin);
+    const int32_t steps = it.sink_tiles + (it.kv_tile_end - it.kv_tile_begin);
+    out.total_steps += steps;
+    out.max_item_steps = std::max(out.max_item_steps, steps);
   }
   if (out.total_steps > (int64_t)INT32_MAX / 2) return fail(SLACK_EINVAL, "batch too large (key-tile steps)");
   out.sparse_steps_off = (out.ws.total + 15) & ~(size_t)15;

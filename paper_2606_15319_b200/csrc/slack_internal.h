@@ -91,6 +91,7 @@ struct HostPlan {
   int32_t mask_rows = 0;        // sum over streams of ceil(q_len / 256)
   int32_t mask_words_min = 1;   // 32-bit words a mask row needs: ceil(max_s ceil(pos_hi / 128) / 32)
   int64_t total_steps = 0;      // sum over items of their dense key-tile steps (entries of the step lists)
+  int32_t max_item_steps = 0;   // longest item (the step lists hold 16-bit step indices)
   size_t sparse_steps_off = 0;  // byte offset of uint16 steps[total_steps] (16-byte aligned, >= ws.total)
   size_t sparse_count_off = 0;  // byte offset of int32 item_steps[n_items]
   size_t sparse_total = 0;      // workspace bytes slack_chunk_attention_sparse needs
