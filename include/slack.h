@@ -214,7 +214,11 @@ slack_status slack_profile_read(slack_ctx *ctx, double *total_ms, int32_t *n_lau
  * instantiation of the kernel that stores clock64() time stamps of CTA 0's first item (rows 0/1 = softmax of query
  * tile 0/1, row 2 = MMA issuer, row 3 = per-warp arrivals; [row][kv step < 64][8 slots], slots documented in
  * csrc/attn_tc.cu) and, from word 2048 on, {clock start, clock end, globaltimer start, end} of every CTA.  NULL switches back to
- * the production instantiation, which contains no trace code. */
+ * the production instantiation, which contains no trace code.
+ * key 2: value != NULL routes dense tensor-core launches of plans made for at most half of the device's SMs
+ * (slack_plan_opts.sm_count <= SMs / 2) to the experimental 2-CTA-cluster kernel (csrc/attn_tc2.cu: one query tile per
+ * SM, double-buffered S, K/V tiles shared by TMA multicast); same results, currently ~6 % slower;
+ * NULL switches back. */
 slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value);
 /* Every in-kernel barrier wait is bounded; a wait that times out records {0xDEAD, block<<32|thread, tag<<32|parity, 0}
  * in host-mapped memory and traps the launch (reported as SLACK_ECUDA by the next call).  This reads that record. */

@@ -291,6 +291,10 @@ class Context:
         """int32 device tensor of 2048 + 4 * n_sm words (or None): clock trace, see include/slack.h."""
         self._check(self.lib.slack_debug_set(self.handle, 1, _ptr(tensor)))
 
+    def debug_use_cluster_kernel(self, on: bool) -> None:
+        """Route dense tensor-core launches of plans made for <= sm_count / 2 queues to the 2-CTA-cluster kernel."""
+        self._check(self.lib.slack_debug_set(self.handle, 2, C.c_void_p(1) if on else None))
+
     def debug_timeout(self):
         buf = (C.c_uint64 * 4)()
         self.lib.slack_debug_timeout(self.handle, buf)

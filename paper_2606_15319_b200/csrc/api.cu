@@ -45,6 +45,8 @@ struct slack_ctx {
   unsigned long long *d_dbg = nullptr;
   float *dbg_s = nullptr;
   uint32_t *dbg_t = nullptr;
+  bool use_cluster_kernel = false; // debug key 2: the 2-CTA-cluster attention kernel (attn_tc2.cu) for dense plans
+  bool tc2_configured = false;
   // per-launch timing of the attention kernel (slack_profile_attention)
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_events; // pairs: [2i] before, [2i+1] after
@@ -101,10 +103,10 @@ slack_status check_pool(slack_ctx *ctx, const slack_pool *pool, const HostPlan *
   return SLACK_OK;
 }
 
-slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t cols, uint64_t rows) {
+slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t cols, uint64_t rows, uint32_t box_rows = 128) {
   const cuuint64_t dims[2] = {cols, rows};
   const cuuint64_t strides[1] = {cols * 2};
-  const cuuint32_t box[2] = {64, 128};
+  const cuuint32_t box[2] = {64, box_rows};
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -192,6 +194,10 @@ slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value) {
   }
   if (key == 1) {
     ctx->dbg_t = reinterpret_cast<uint32_t *>(value);
+    return SLACK_OK;
+  }
+  if (key == 2) {
+    ctx->use_cluster_kernel = value != nullptr;
     return SLACK_OK;
   }
   return set_err(ctx, SLACK_EINVAL, "unknown debug key");
@@ -534,8 +540,14 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   CUtensorMap tm_q, tm_k, tm_v;
   const uint64_t pool_rows = (uint64_t)hp.n_pages * hp.n_heads * hp.page_size;
   if ((st = make_map(ctx, &tm_q, q, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
-  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
-  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  const bool cluster2 = ctx->use_cluster_kernel && !block_mask && 2 * hp.n_cta <= ctx->sm_count;
+  const uint32_t kv_box_rows = cluster2 ? 64 : 128; // the cluster kernel loads half a key tile per CTA
+  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows, kv_box_rows)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows, kv_box_rows)) != SLACK_OK) return st;
+  if (cluster2 && !ctx->tc2_configured) {
+    SLACK_CUDA(ctx, attn_tc2_configure());
+    ctx->tc2_configured = true;
+  }
   TcParams p{};
   p.items = plan->d_items;
   p.cta_begin = plan->d_cta_begin;
@@ -573,7 +585,10 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
     SLACK_CUDA(ctx, cudaEventRecord(ctx->prof_events[2 * ctx->prof_used], cs));
     ev_after = ctx->prof_events[2 * ctx->prof_used + 1];
   }
-  SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
+  if (cluster2)
+    SLACK_CUDA(ctx, launch_attn_tc2(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
+  else
+    SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
   if (ev_after) {
     SLACK_CUDA(ctx, cudaEventRecord(ev_after, cs));
     ctx->prof_used++;
