@@ -20,7 +20,12 @@
 // 128-key step, no less than the ~1640 the two-tile kernel needs per tile-step; the SM's softmax instruction throughput,
 // not the pipeline shape, is the limit.  Two variants measured on top of it did worse: two fully
 // independent column streams with their own O accumulators and no per-step exchange (-12 %), and prefetching S of the
-// next step into registers (S_{j+1} completes only ~1000 cycles into step j: -25 %).
+// next step into registers (S_{j+1} completes only ~1000 cycles into step j: -25 %).  The number of threads per query row
+// was also varied on this pipeline, where the softmax never waits: 1 thread per row (4 softmax warps, 128 columns each)
+// 6.08 M cycles, 2 per row (this file) 5.37 M, 4 per row (16 warps, 32 columns each, 128-thread barrier) 5.7 M.  One warp
+// alone on a sub-partition needs ~1980 cycles per 128 x 128 tile step whether or not anything else runs beside it (it is
+// latency-bound: a third of its time is fixed-latency dependency stalls), a sub-partition overlaps two such warps almost
+// perfectly, and that is what the two-tile kernel already does.
 //
 // CTA = 384 threads: warp 0 TMA producer, warp 1 MMA issuer, warps 2-3 idle, warps 4-7 softmax of key columns 0..63,
 // warps 8-11 of columns 64..127 (thread = query row = TMEM lane).  Both CTAs of a cluster walk the same planned queue
