@@ -25,7 +25,10 @@
 // 6.08 M cycles, 2 per row (this file) 5.37 M, 4 per row (16 warps, 32 columns each, 128-thread barrier) 5.7 M.  One warp
 // alone on a sub-partition needs ~1980 cycles per 128 x 128 tile step whether or not anything else runs beside it (it is
 // latency-bound: a third of its time is fixed-latency dependency stalls), a sub-partition overlaps two such warps almost
-// perfectly, and that is what the two-tile kernel already does.
+// perfectly, and that is what the two-tile kernel already does.  Finally, a what-if build of this file WITHOUT the exponentials
+// still needs 5.31 M cycles: the bound here is not the softmax arithmetic but (most likely) the shared-memory port: every
+// SM ingests the whole K/V tile (64 KB per step) and the SS-mode MMAs read 98 KB of operands per step, 162 KB per 1024
+// MMA cycles at 128 B/clk.  The remedy is cta_group::2 (each CTA stores and feeds half of every K/V tile).
 //
 // CTA = 384 threads: warp 0 TMA producer, warp 1 MMA issuer, warps 2-3 idle, warps 4-7 softmax of key columns 0..63,
 // warps 8-11 of columns 64..127 (thread = query row = TMEM lane).  Both CTAs of a cluster walk the same planned queue
