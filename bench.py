@@ -338,18 +338,19 @@ def run_ours(args):
 
     # ---- device-resident timing (value) + per-kernel roofline ------------------------------------------------------
     sampler = ClockSampler(local) if rank == 0 else None
-    ctx.profile_attention(True)
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
-    ctx.profile_read()
-    ms = timed(step, args.steps, 0)
-    k_ms, k_n = ctx.profile_read()
-    ctx.profile_attention(False)
-    clocks = sampler.stop() if sampler else None
+    ms = timed(step, args.steps, 0)                   # the timed region of `value`: no profiling events in the stream
     launches = state["launches"]
     plan_ms = 1e3 * state["plan_s"] / args.steps
     value = world * flops_step * args.steps / (ms * 1e-3) / 1e12
+    # the same K steps once more with the library's event pair around every attention kernel (roofline figure)
+    ctx.profile_attention(True)
+    ms_prof = timed(step, args.steps, 0)
+    k_ms, k_n = ctx.profile_read()
+    ctx.profile_attention(False)
+    clocks = sampler.stop() if sampler else None
 
     # ---- end to end: inputs from pinned host memory, output read back, inside the timed region ----------------------
     e2e = None
@@ -461,7 +462,7 @@ def run_ours(args):
                     "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6500 GB/s",
                     "kernel_ms_avg": kernel_ms, "launches_timed": k_n, "bytes_per_launch": bytes_layer,
                     "flops_per_byte": intensity, "ridge_flops_per_byte": peak * 1e12 / (hbm_peak * 1e9),
-                    "tflops": achieved, "kernel_share_of_step": (k_ms / ms) if k_n else None}
+                    "tflops": achieved, "kernel_share_of_step": (k_ms / ms_prof) if k_n else None}
     else:
         roofline = {"bound": "tensor", "kernel": "attn_tc_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                     "frac": (achieved / peak) if achieved else None,
@@ -470,7 +471,7 @@ def run_ours(args):
                     "flops_per_launch": flops_layer,
                     "frac_of_burst": (achieved / float(peaks["bf16_tflops"])) if achieved and "bf16_tflops" in peaks else None,
                     "frac_of_nominal_2250": (achieved / 2250.0) if achieved else None,
-                    "kernel_share_of_step": (k_ms / ms) if k_n else None}
+                    "kernel_share_of_step": (k_ms / ms_prof) if k_n else None}
 
     # ---- CPU baseline: the oracle on layer 0 of this very run (also a live parity spot check) ----------------------
     cpu = None

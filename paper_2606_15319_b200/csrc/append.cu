@@ -15,6 +15,8 @@ __global__ void __launch_bounds__(kAppendThreads)
 kv_append_kernel(const uint4 *__restrict__ k_new, const uint4 *__restrict__ v_new, uint4 *__restrict__ k_pool,
                  uint4 *__restrict__ v_pool, const DevStream *__restrict__ streams,
                  const int32_t *__restrict__ page_tables, int n_heads, int page_log2, int vec_log2 /* log2(16-byte vectors per (token, head) row) */) {
+  pdl_wait(); // K_new / V_new may come from the kernel before; the pool may still be read by the previous layer's attention
+  pdl_launch_dependents();
   const DevStream s = streams[blockIdx.y];
   if (s.q_len == 0) return;
   const int vecs = 1 << vec_log2;
@@ -74,11 +76,11 @@ cudaError_t launch_kv_append(const void *k_new, const void *v_new, void *k_pool,
   if (cap < 1) cap = 1;
   const int gx = (int)(want < cap ? want : cap);
   dim3 grid(gx > 0 ? gx : 1, n_streams);
-  kv_append_kernel<<<grid, kAppendThreads, 0, st>>>(
-      reinterpret_cast<const uint4 *>(k_new), reinterpret_cast<const uint4 *>(v_new), reinterpret_cast<uint4 *>(k_pool),
-      reinterpret_cast<uint4 *>(v_pool), d_streams, d_page_tables, n_heads, ilog2(page_size), ilog2(vecs));
+  cudaError_t e = launch_pdl(kv_append_kernel, grid, dim3(kAppendThreads), 0, st, reinterpret_cast<const uint4 *>(k_new),
+                             reinterpret_cast<const uint4 *>(v_new), reinterpret_cast<uint4 *>(k_pool),
+                             reinterpret_cast<uint4 *>(v_pool), d_streams, d_page_tables, n_heads, ilog2(page_size), ilog2(vecs));
   if (n_launched) *n_launched += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 } // namespace slack

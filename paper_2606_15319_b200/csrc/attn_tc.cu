@@ -166,6 +166,10 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_smem));
+  // PDL: everything above (barrier init, TMEM allocation, descriptor prefetch) overlapped the previous kernel's drain;
+  // from here on the kernel reads memory its predecessors wrote (pool, Q, step lists) and writes Out / the workspace
+  pdl_wait();
+  pdl_launch_dependents();
 
   const int H = p.n_heads;
   const int P = 1 << p.page_log2;
@@ -592,14 +596,15 @@ cudaError_t attn_tc_configure() {
 
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched) {
+  cudaError_t e;
   if (p.steps != nullptr)
-    attn_tc_kernel<false, true><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+    e = launch_pdl(attn_tc_kernel<false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   else if (p.dbg_t != nullptr)
-    attn_tc_kernel<true, false><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+    e = launch_pdl(attn_tc_kernel<true, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   else
-    attn_tc_kernel<false, false><<<n_cta, kTcThreads, kSmemBytes, st>>>(p, tm_q, tm_k, tm_v);
+    e = launch_pdl(attn_tc_kernel<false, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   if (n_launched) *n_launched += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 } // namespace slack

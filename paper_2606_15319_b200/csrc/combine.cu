@@ -22,6 +22,8 @@ __global__ void __launch_bounds__(kCombineThreads)
 combine_kernel(const DevCombine *__restrict__ combines, const float *__restrict__ ws_o, const float *__restrict__ ws_lse,
                __nv_bfloat16 *__restrict__ out, float *__restrict__ lse, int n_heads, int total_q) {
   static_assert(D == 128, "one float4 per lane");
+  pdl_wait(); // the partials are written by the attention kernel right before
+  pdl_launch_dependents();
   const DevCombine cb = combines[blockIdx.x];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r = blockIdx.y * kRowsPerCta + warp;
@@ -83,10 +85,10 @@ cudaError_t launch_combine(const DevCombine *d_combines, int n_combines, const f
                            float *lse, int n_heads, int head_dim, int total_q, cudaStream_t st, int *n_launched) {
   if (n_combines == 0) return cudaSuccess;
   if (head_dim != 128) return cudaErrorInvalidValue;
-  combine_kernel<128><<<dim3((unsigned)n_combines, kItemRows / kRowsPerCta), kCombineThreads, 0, st>>>(d_combines, ws_o, ws_lse,
-                                                              reinterpret_cast<__nv_bfloat16 *>(out), lse, n_heads, total_q);
+  cudaError_t e = launch_pdl(combine_kernel<128>, dim3((unsigned)n_combines, kItemRows / kRowsPerCta), dim3(kCombineThreads), 0, st,
+                             d_combines, ws_o, ws_lse, reinterpret_cast<__nv_bfloat16 *>(out), lse, n_heads, total_q);
   if (n_launched) *n_launched += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 } // namespace slack

@@ -7,6 +7,34 @@
 
 namespace slack {
 
+// Programmatic dependent launch (PDL): kernels of the per-layer hot loop (append -> attention -> combine, layer after
+// layer on one stream) are launched with cudaLaunchAttributeProgrammaticStreamSerialization so that a kernel's launch
+// overlaps the drain of its predecessor (~5-7 us per boundary, 3 boundaries per layer).  Every such kernel calls
+// pdl_wait() before it touches memory a predecessor may still be writing (it returns once all prerequisite grids have
+// completed and flushed), and pdl_launch_dependents() right after so that its own successor can be staged early.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+#ifdef SLACK_NO_PDL
+  cfg.numAttrs = 0; // A/B switch: plain stream-ordered launches
+#else
+  cfg.numAttrs = 1;
+#endif
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 // A1: paged scatter copy. elem_bytes = 2 (bf16) or 4 (f32). Launches 1 kernel (0 if nothing to copy).
 cudaError_t launch_kv_append(const void *k_new, const void *v_new, void *k_pool, void *v_pool, const DevStream *d_streams,
                              int n_streams, int max_q_len, const int32_t *d_page_tables, int n_heads, int head_dim,

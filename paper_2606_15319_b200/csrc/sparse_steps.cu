@@ -19,6 +19,8 @@ constexpr int kStepsThreads = 128;
 __global__ void __launch_bounds__(kStepsThreads)
 sparse_steps_kernel(const DevItem *__restrict__ items, int n_items, const uint32_t *__restrict__ mask, int n_heads,
                     int mask_words, uint16_t *__restrict__ steps, int32_t *__restrict__ count) {
+  pdl_wait(); // the mask may be produced by the kernel before; the step lists may still be read by the previous attention
+  pdl_launch_dependents();
   const int k = blockIdx.x * (kStepsThreads / 32) + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (k >= n_items) return;
@@ -47,10 +49,10 @@ cudaError_t launch_sparse_steps(const DevItem *d_items, int n_items, const uint3
                                 uint16_t *steps, int32_t *count, cudaStream_t st, int *n_launched) {
   if (n_items == 0) return cudaSuccess;
   const int wpb = kStepsThreads / 32;
-  sparse_steps_kernel<<<(unsigned)((n_items + wpb - 1) / wpb), kStepsThreads, 0, st>>>(d_items, n_items, mask, n_heads,
-                                                                                      mask_words, steps, count);
+  cudaError_t e = launch_pdl(sparse_steps_kernel, dim3((unsigned)((n_items + wpb - 1) / wpb)), dim3(kStepsThreads), 0, st, d_items,
+                             n_items, mask, n_heads, mask_words, steps, count);
   if (n_launched) *n_launched += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 } // namespace slack
