@@ -346,10 +346,11 @@ def run_ours(args):
     plan_ms = 1e3 * state["plan_s"] / args.steps
     value = world * flops_step * args.steps / (ms * 1e-3) / 1e12
     # the same K steps once more with the library's event pair around every attention kernel (roofline figure)
-    ctx.profile_attention(True)
+    ctx.profile_enable(binding.PROF_ATTENTION)
     ms_prof = timed(step, args.steps, 0)
-    k_ms, k_n = ctx.profile_read()
-    ctx.profile_attention(False)
+    k_list = ctx.profile_read(binding.PROF_ATTENTION)
+    k_ms, k_n = float(sum(k_list)), len(k_list)
+    ctx.profile_enable(0)
     clocks = sampler.stop() if sampler else None
 
     # ---- end to end: inputs from pinned host memory, output read back, inside the timed region ----------------------

@@ -17,15 +17,22 @@
  *     lse_i   = ln sum_{t in visible} exp(scale * <q_i, k_t>)
  *
  * Token -> slot rule (the single source of truth for "page-table indexing"):
- *     logical token t of a stream lives at physical page  page_table[(base + t) / page_size],
- *     slot (base + t) % page_size, i.e. element offset ((page * n_heads + h) * page_size + slot) * head_dim + d
- *     of a pool tensor laid out [n_pages][n_heads][page_size][head_dim] (head_dim contiguous).
+ *     held token t of a stream sits at POSITION pos(t) = base + t (+ gap_slots if t >= sink_len; see slack_stream),
+ *     i.e. at physical page  page_table[pos / page_size], slot pos % page_size, element offset
+ *     ((page * n_heads + h) * page_size + slot) * head_dim + d of a pool tensor laid out
+ *     [n_pages][n_heads][page_size][head_dim] (head_dim contiguous).
  *
  * Ownership: every device buffer (pools, q, k_new, v_new, out, lse, workspace) is CALLER-owned.  The library owns
- * only the context, plans and their small device-side tables.  Host descriptor arrays (slack_stream, page tables)
- * are read during the call only.  All device work is enqueued on the caller's CUDA stream; no call synchronises the
- * device except slack_plan (one small upload, synchronous) and slack_destroy / slack_plan_destroy.
+ * only the context, plans and their small device-side tables, which live in a ctx-owned arena (device memory plus a
+ * pinned host mirror, allocated once and grown rarely).  Host descriptor arrays (slack_stream, page tables) are read
+ * during the call only.  All device work is enqueued on the caller's CUDA stream.  No call synchronises the device
+ * except slack_destroy: slack_plan uploads its tables on a private stream and the first launch that uses the plan waits
+ * for that copy ON THE DEVICE; slack_plan_destroy and the staging of slack_kv_append / slack_kv_transfer hand their
+ * arena blocks back through CUDA events recorded behind the last kernel that reads them.  A CUDA stream a plan was
+ * used on must outlive the plan.
  * Errors: every call returns a slack_status and never aborts, throws or prints; slack_last_error() gives a text.
+ * Every in-kernel barrier wait is bounded: a wait that times out traps the launch, the next call reports SLACK_ECUDA
+ * and its text names the block, thread and barrier that gave up.
  * A context is not thread-safe; plans are immutable after creation.
  * There is NO CPU fallback: without a CUDA device only host-only contexts (device = -1) exist, and they can plan
  * (for inspection) but every data-path call on them returns SLACK_ECUDA.
@@ -40,7 +47,7 @@
 extern "C" {
 #endif
 
-#define SLACK_ABI_VERSION 1
+#define SLACK_ABI_VERSION 2
 
 typedef enum {
   SLACK_OK = 0,
@@ -74,9 +81,16 @@ typedef struct {
   int32_t base;              /* slot of logical token 0 inside page_table[0]; 0 <= base < page_size             */
   int32_t window;            /* Wt: max visible keys INCLUDING the own chunk; 0 = unlimited              */
   int32_t sink_len;          /* "sink + local": the first sink_len tokens stay visible when the window has
-                                moved past them: visible = [0, sink) U [max(sink, lo), n); 0 = no sink; their pages
-                                must still be listed in page_table                                                */
-  int32_t n_table_pages;     /* >= ceil((base + Lc + Lq) / page_size)                                           */
+                                moved past them: visible = [0, sink) U [max(sink, lo), n); 0 = no sink            */
+  int32_t gap_slots;         /* unused slots between the end of the sink and the first held token behind it: token
+                                t >= sink_len lives at position base + gap_slots + t (t < sink_len: base + t).  This is
+                                how tokens that left the window are DROPPED from a sink stream ("keeps KV entries
+                                only for the most recent W chunks"): they vanish from the numbering, cache_len counts
+                                held tokens only, their whole pages leave the table, and the cache stays bounded
+                                however long the stream runs.  0 = contiguous.  Needs sink_len > 0 and
+                                cache_len >= sink_len when non-zero                                                */
+  int32_t n_table_pages;     /* >= ceil((base + gap_slots + Lc + Lq) / page_size)                               */
+  int32_t reserved;          /* 0                                                                                */
   const int32_t *page_table; /* HOST: logical page -> physical page id in [0, n_pages)                          */
 } slack_stream;
 
@@ -101,7 +115,7 @@ typedef struct {
   int32_t q_rows;        /* valid rows, 1..256 (two 128-row MMA tiles)                                           */
   int32_t kv_tile_begin; /* [begin, end) in position-tile units                                                  */
   int32_t kv_tile_end;
-  int32_t pos_lo;        /* visible positions [pos_lo, pos_hi) = [base + lo, base + n)                           */
+  int32_t pos_lo;        /* visible positions [pos_lo, pos_hi) = [pos(lo), pos(n-1) + 1)                         */
   int32_t pos_hi;
   int32_t sink_tiles;    /* tiles of the sink [base, sink_pos_hi) visited BEFORE the window tiles (0: none; only the
                             first piece of a split row carries them), starting at tile base / 128                  */
@@ -130,9 +144,10 @@ slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, c
 
 /* ---- A2: plan (host) ---------------------------------------------------------------------------------------- */
 /* Validates the batch, cuts it into (stream, head, q-tile, kv-tile-range) work items, balances them over the SMs
- * (split-KV where a key range is cut), builds the combine list and uploads the tables (one synchronous copy).  The
- * plan depends only on (q_len, cache_len, base, window, page_table, n_heads, head_dim, page_size, dtype): it is valid
- * for every layer and denoising step of the chunk batch (same page ids in every layer's pool). */
+ * (split-KV where a key range is cut), builds the combine list and uploads the tables (asynchronous, see "Ownership").
+ * The plan depends only on the stream descriptors and (n_heads, head_dim, page_size, dtype): it is valid for every
+ * layer and denoising step of the chunk batch (same page ids in every layer's pool).  slack_plan_destroy never blocks;
+ * it may be called before or after slack_destroy of the plan's context. */
 slack_status slack_plan(slack_ctx *ctx, const slack_pool *pool_shape, int32_t n_streams,
                         const slack_stream *streams, const slack_plan_opts *opts, slack_plan_t **plan);
 void slack_plan_destroy(slack_plan_t *plan);
@@ -156,7 +171,7 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
 /* PAPER.md P:88 knob (2): "skips nonselected attention blocks with sparse masks", controlled by the attention sparsity
  * rho in {0, .6, .7, .8, .9}.  The block-SELECTION rule is Light Forcing's and not part of this path:
  * the mask is an input.  Semantics: query row i of a stream (chunk-local) belongs to query block i / 256; key token t
- * belongs to key block (base + t) / 128 (the 128-position key tiles of slack_work_item); row i uses key t iff t is
+ * belongs to key block pos(t) / 128 (its position, see the token -> slot rule; the 128-position key tiles of slack_work_item); row i uses key t iff t is
  * visible (window / sink, as in slack_chunk_attention) AND its key block is selected for (query block, head).  A row
  * that is left without any key gets out = 0 and lse = -inf.
  * block_mask: DEVICE uint32 [slack_plan_mask_rows(plan)][n_heads][mask_words]; mask row r = the r-th 256-row query block
@@ -173,7 +188,7 @@ slack_status slack_chunk_attention_sparse(slack_ctx *ctx, const slack_plan_t *pl
                                           int32_t mask_words, void *workspace, size_t workspace_bytes, void *cuda_stream);
 size_t slack_plan_sparse_workspace_bytes(const slack_plan_t *plan);
 int32_t slack_plan_mask_rows(const slack_plan_t *plan);      /* sum over streams of ceil(q_len / 256)                 */
-int32_t slack_plan_mask_min_words(const slack_plan_t *plan); /* ceil(max over streams of ceil((base+Lc+Lq)/128) / 32) */
+int32_t slack_plan_mask_min_words(const slack_plan_t *plan); /* ceil(max over streams of ceil(end position / 128) / 32) */
 
 /* ---- state-plane page transfer -------------------------------------------------------------- */
 /* PAPER.md P:255 "transfer(stream, src, dst, page_range)": the single primitive behind credit-aware eviction,
@@ -191,7 +206,8 @@ int32_t slack_plan_mask_min_words(const slack_plan_t *plan); /* ceil(max over st
  * src_page_ids / dst_page_ids: HOST int32[n_pages], read during the call; destination ids must be distinct.  The
  * caller's page tables are its own business: after the transfer the stream's table on the destination side is
  * dst_page_ids in the same logical order.  Errors: SLACK_EINVAL for ids out of range, duplicate destinations, mismatched
- * shapes or an empty head range. */
+ * shapes, an empty head range, or - when a layer's source and destination are the same pool - a page that is both
+ * read and written by the call (the copies of one launch are unordered). */
 slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_pool *src_pools, const slack_pool *dst_pools,
                                int32_t n_pages, const int32_t *src_page_ids, const int32_t *dst_page_ids,
                                int32_t head_begin, int32_t head_end, void *cuda_stream, void *const *layer_done_events);
@@ -199,30 +215,53 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
 /* Number of kernels the last slack_chunk_attention / slack_kv_append call on this ctx launched (bench bookkeeping). */
 int32_t slack_last_launch_count(const slack_ctx *ctx);
 
-/* ---- measurement (bench.py's roofline figure) ------------------------------------------------------- */
-/* enable != 0: every following slack_chunk_attention records a CUDA event pair on the caller's stream directly
- * around the tensor-core attention kernel (not the combine kernel).  slack_profile_read waits for the recorded pairs,
- * returns the summed kernel time in milliseconds and the number of launches timed, and resets the record.  Off by
- * default: the events cost two stream operations per call. */
-slack_status slack_profile_attention(slack_ctx *ctx, int32_t enable);
-slack_status slack_profile_read(slack_ctx *ctx, double *total_ms, int32_t *n_launches);
+/* ---- A0 + A5: page bookkeeping of one worker's pool (host only, integers only) -------------------------------- */
+/* the K/V of all streams on a worker live in one paged pool "mapped to physical pages through a logical
+ * page table, avoiding fragmentation"; every finished chunk is "appended to a rolling KV cache for subsequent
+ * chunks"; the cache "preserves the first few chunks as a global sink and keeps KV entries only for the most
+ * recent W chunks".  A slack_cache_t does exactly that bookkeeping for the page ids of ONE pool shape (the same ids
+ * index every layer's pool): a free list, one page table per stream, the commit Lc += Lq, and the release of pages that
+ * left the window.  It owns no device memory and makes no CUDA call.
+ *
+ *   slack_cache_open        new stream with its window Wt (tokens, 0 = unlimited) and sink length; no page yet
+ *   slack_cache_begin_chunk A0: first drops what the window of the chunk about to be generated no longer covers
+ *                           (lo = max(sink, Lc + q_len - Wt)): pages that hold no visible position go back to the free
+ *                           list UNCLEARED, and the dropped tokens leave the numbering (cache_len, base or gap_slots
+ *                           shrink accordingly; policy below); then takes pages from the free list until the table
+ *                           covers [0, Lc + q_len); fills *desc, ready for slack_plan / slack_kv_append.
+ *                           desc->page_table points into the cache and stays valid until the next call that names this
+ *                           stream.  Calling it again before the commit with the same q_len returns the same descriptor
+ *                           (the S denoising steps of a chunk re-append and re-attend with one descriptor).
+ *                           SLACK_ENOMEM when the free list runs dry (nothing is taken in that case).
+ *   slack_cache_commit      A5: the chunk is final: Lc += q_len.
+ *   slack_cache_close       all pages of the stream go back to the free list.
+ * trim_policy: SLACK_TRIM_PAGES drops whole pages only (the first held token is then the first slot of a page or the
+ * stream's old start; `window` clips the rest inside the kernel); SLACK_TRIM_TOKENS also drops the invisible tokens at the
+ * head of the first kept page (base, or gap_slots for a sink stream, walks through the page).  Both give identical
+ * attention results.  Freed pages are handed out again most-recently-freed first. */
+typedef struct slack_cache_s slack_cache_t; /* opaque */
+typedef enum { SLACK_TRIM_PAGES = 0, SLACK_TRIM_TOKENS = 1 } slack_trim_policy;
+slack_status slack_cache_create(int32_t n_pages, int32_t page_size, int32_t trim_policy, slack_cache_t **cache);
+void slack_cache_destroy(slack_cache_t *cache);
+slack_status slack_cache_open(slack_cache_t *cache, int32_t window, int32_t sink_len, int32_t *stream_id);
+slack_status slack_cache_begin_chunk(slack_cache_t *cache, int32_t stream_id, int32_t q_len, slack_stream *desc);
+slack_status slack_cache_commit(slack_cache_t *cache, int32_t stream_id);
+slack_status slack_cache_close(slack_cache_t *cache, int32_t stream_id);
+int32_t slack_cache_free_pages(const slack_cache_t *cache);
+int32_t slack_cache_stream_pages(const slack_cache_t *cache, int32_t stream_id); /* pages the stream holds; -1: no such stream */
+const char *slack_cache_last_error(const slack_cache_t *cache);
 
-/* ---- diagnostics (never on the data path) ---------------------------------------------------------------------- */
-/* key 0: `value` = DEVICE pointer to a [2][128][128] fp32 buffer that receives the first two S = QK^T tiles computed by
- * CTA 0 of the next tensor-core launches (NULL switches the dump off).
- * key 1: `value` = DEVICE pointer to a uint32 buffer of 2048 + 4 * (number of SMs) words; while set, tensor-core launches use a diagnostic
- * instantiation of the kernel that stores clock64() time stamps of CTA 0's first item (rows 0/1 = softmax of query
- * tile 0/1, row 2 = MMA issuer, row 3 = per-warp arrivals; [row][kv step < 64][8 slots], slots documented in
- * csrc/attn_tc.cu) and, from word 2048 on, {clock start, clock end, globaltimer start, end} of every CTA.  NULL switches back to
- * the production instantiation, which contains no trace code.
- * key 2: value != NULL routes dense tensor-core launches of plans made for at most half of the device's SMs
- * (slack_plan_opts.sm_count <= SMs / 2) to the experimental 2-CTA-cluster kernel (csrc/attn_tc2.cu: one query tile per
- * SM, double-buffered S, K/V tiles shared by TMA multicast); same results, currently ~6 % slower;
- * NULL switches back. */
-slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value);
-/* Every in-kernel barrier wait is bounded; a wait that times out records {0xDEAD, block<<32|thread, tag<<32|parity, 0}
- * in host-mapped memory and traps the launch (reported as SLACK_ECUDA by the next call).  This reads that record. */
-slack_status slack_debug_timeout(slack_ctx *ctx, uint64_t out[4]);
+/* ---- measurement (bench.py's per-kernel figures) --------------------------------------------------- */
+/* slack_profile_enable: `kinds` = OR of SLACK_PROF_*; while a kind is enabled every launch of that kernel is bracketed
+ * by a CUDA event pair on the caller's stream.  slack_profile_read waits for the recorded pairs of one kind, copies up
+ * to `capacity` per-launch durations (milliseconds, launch order) to `ms`, stores the number recorded in *n_launches and
+ * resets that kind's record.  Measurement only: the events cost two stream operations per launch and switch off the
+ * programmatic-dependent-launch overlap around the bracketed kernel. */
+#define SLACK_PROF_ATTENTION 1 /* the attention kernel (not its combine)  */
+#define SLACK_PROF_APPEND 2    /* the KV append kernel                    */
+#define SLACK_PROF_COMBINE 4   /* the split-KV combine kernel             */
+slack_status slack_profile_enable(slack_ctx *ctx, int32_t kinds);
+slack_status slack_profile_read(slack_ctx *ctx, int32_t kind, double *ms, int32_t capacity, int32_t *n_launches);
 
 #ifdef __cplusplus
 }

@@ -22,14 +22,16 @@ Definition; for stream s, head h, with n = Lc + Lq:
     s_t     = scale * <q_i, k_t>      for t in visible   (every query row sees every visible key:
                                                           bidirectional inside the own chunk, A1)
     out_i   = sum_t softmax_t(s)_t * v_t ,   lse_i = ln sum_t exp(s_t)
-Token t of a stream lives at physical page page_table[(base+t) // P], slot (base+t) % P of a pool
-laid out [n_pages][H][P][D] (the token->slot rule of include/slack.h).
+Held token t of a stream sits at POSITION pos(t) = base + t, plus gap_slots when t >= sink_len (the hole
+left behind the sink by tokens that were dropped from a bounded "sink + local" cache), i.e. at
+physical page page_table[pos // P], slot pos % P of a pool laid out [n_pages][H][P][D] (the
+token->slot rule of include/slack.h).  cache_len counts held tokens only.
 
 Block-sparse variant (PAPER.md P:88 knob (2) "skips nonselected attention blocks
 with sparse masks ... controlled by attention sparsity rho", rho in {0,.6,.7,.8,.9} P:568, selection
 rule from Light Forcing [39] P:319 - the rule is NOT in the paper, so the mask is an INPUT here):
     query block  qb = i // block_q            (i = chunk-local query row)
-    key block    kb = (base + t) // block_k   (position of key token t in the stream's page-table space)
+    key block    kb = pos(t) // block_k       (position of key token t in the stream's page-table space)
     t is used iff it is visible (above) AND mask[h, qb, kb]
     out_i = softmax over the used keys; a row with no used key has out_i = 0 and lse_i = -inf.
 
@@ -78,9 +80,16 @@ def to_f64(x: np.ndarray, dtype: str) -> np.ndarray:
 # token -> slot rule and visible range
 # ----------------------------------------------------------------------------------------------
 
+def token_positions(stream, tokens: np.ndarray) -> np.ndarray:
+    """pos(t) = base + t for the sink tokens t < sink_len, base + gap_slots + t behind them (include/slack.h)."""
+    t = np.asarray(tokens, dtype=np.int64)
+    gap = getattr(stream, "gap_slots", 0)
+    return stream.base + t + np.where(t >= getattr(stream, "sink_len", 0), gap, 0)
+
+
 def token_slots(stream, tokens: np.ndarray, page_size: int) -> Tuple[np.ndarray, np.ndarray]:
-    """(physical page, slot) of logical tokens of one stream: page_table[(base+t)//P], (base+t)%P."""
-    pos = stream.base + np.asarray(tokens, dtype=np.int64)
+    """(physical page, slot) of held tokens of one stream: page_table[pos // P], pos % P."""
+    pos = token_positions(stream, tokens)
     table = np.asarray(stream.page_table, dtype=np.int64)
     return table[pos // page_size], pos % page_size
 
@@ -155,7 +164,7 @@ def _sparse_stream(k_pool, v_pool, s, toks, sel, q, row0, scale, dtype, mask, bl
     """Block-sparse rows of one stream: for every head and query block, softmax over the visible keys whose
     key block is selected (header; P:88 knob (2)).  Rows of one query block share their key set."""
     n_heads = q.shape[1]
-    key_block = (s.base + toks) // block_k                 # key block of every visible token
+    key_block = token_positions(s, toks) // block_k        # key block of every visible token
     assert mask.shape[0] == n_heads and mask.shape[1] >= -(-s.q_len // block_q) and mask.shape[2] > int(key_block.max())
     for h in range(n_heads):
         for qb in np.unique(sel // block_q):

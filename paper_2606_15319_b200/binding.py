@@ -34,7 +34,8 @@ class CPool(C.Structure):
 
 class CStream(C.Structure):
     _fields_ = [("q_len", C.c_int32), ("cache_len", C.c_int32), ("base", C.c_int32), ("window", C.c_int32),
-                ("sink_len", C.c_int32), ("n_table_pages", C.c_int32), ("page_table", C.POINTER(C.c_int32))]
+                ("sink_len", C.c_int32), ("gap_slots", C.c_int32), ("n_table_pages", C.c_int32), ("reserved", C.c_int32),
+                ("page_table", C.POINTER(C.c_int32))]
 
 
 class CPlanOpts(C.Structure):
@@ -71,11 +72,22 @@ SYMBOLS = {
     "slack_plan_mask_min_words": (C.c_int32, [_VP]),
     "slack_kv_transfer": (C.c_int, [_VP, C.c_int32, C.POINTER(CPool), C.POINTER(CPool), C.c_int32, C.POINTER(C.c_int32),
                                    C.POINTER(C.c_int32), C.c_int32, C.c_int32, _VP, C.POINTER(_VP)]),
-    "slack_profile_attention": (C.c_int, [_VP, C.c_int32]),
-    "slack_profile_read": (C.c_int, [_VP, C.POINTER(C.c_double), C.POINTER(C.c_int32)]),
-    "slack_debug_set": (C.c_int, [_VP, C.c_int32, _VP]),
-    "slack_debug_timeout": (C.c_int, [_VP, C.POINTER(C.c_uint64)]),
+    "slack_profile_enable": (C.c_int, [_VP, C.c_int32]),
+    "slack_profile_read": (C.c_int, [_VP, C.c_int32, C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_int32)]),
+    "slack_cache_create": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(_VP)]),
+    "slack_cache_destroy": (None, [_VP]),
+    "slack_cache_open": (C.c_int, [_VP, C.c_int32, C.c_int32, C.POINTER(C.c_int32)]),
+    "slack_cache_begin_chunk": (C.c_int, [_VP, C.c_int32, C.c_int32, C.POINTER(CStream)]),
+    "slack_cache_commit": (C.c_int, [_VP, C.c_int32]),
+    "slack_cache_close": (C.c_int, [_VP, C.c_int32]),
+    "slack_cache_free_pages": (C.c_int32, [_VP]),
+    "slack_cache_stream_pages": (C.c_int32, [_VP, C.c_int32]),
+    "slack_cache_last_error": (C.c_char_p, [_VP]),
 }
+# include/slack_diag.h: only a library built with -DSLACK_DIAGNOSTICS exports these
+DIAG_SYMBOLS = {"slack_debug_set": (C.c_int, [_VP, C.c_int32, _VP])}
+PROF_ATTENTION, PROF_APPEND, PROF_COMBINE = 1, 2, 4
+TRIM_PAGES, TRIM_TOKENS = 0, 1
 
 _lib = None
 
@@ -91,19 +103,23 @@ def load() -> C.CDLL:
         for name, (res, args) in SYMBOLS.items():
             fn = getattr(lib, name)
             fn.restype, fn.argtypes = res, args
+        for name, (res, args) in DIAG_SYMBOLS.items():
+            if hasattr(lib, name):
+                fn = getattr(lib, name)
+                fn.restype, fn.argtypes = res, args
         _lib = lib
     return _lib
 
 
 def _stream_array(streams: Sequence):
-    """slack_stream[] from StreamSpec-like objects (q_len, cache_len, base, window, sink_len, page_table)."""
+    """slack_stream[] from StreamSpec-like objects (q_len, cache_len, base, window, sink_len, gap_slots, page_table)."""
     arr = (CStream * max(len(streams), 1))()
     keep = []
     for i, s in enumerate(streams):
         table = np.ascontiguousarray(s.page_table, dtype=np.int32)
         keep.append(table)
         arr[i] = CStream(int(s.q_len), int(s.cache_len), int(s.base), int(s.window), int(getattr(s, "sink_len", 0)),
-                         int(table.size), table.ctypes.data_as(C.POINTER(C.c_int32)))
+                         int(getattr(s, "gap_slots", 0)), int(table.size), 0, table.ctypes.data_as(C.POINTER(C.c_int32)))
     return arr, keep
 
 
@@ -274,31 +290,84 @@ class Context:
                                                int(head_begin), int(head_end), _cuda_stream(stream), ev))
 
     # --- measurement ---------------------------------------------------------------------------------------------------
-    def profile_attention(self, enable: bool) -> None:
-        self._check(self.lib.slack_profile_attention(self.handle, int(bool(enable))))
+    def profile_enable(self, kinds: int) -> None:
+        """kinds: OR of PROF_ATTENTION / PROF_APPEND / PROF_COMBINE (0 = off); see include/slack.h."""
+        self._check(self.lib.slack_profile_enable(self.handle, int(kinds)))
 
-    def profile_read(self):
-        """(total milliseconds, launches) of the attention kernel since the last read."""
-        ms, n = C.c_double(0), C.c_int32(0)
-        self._check(self.lib.slack_profile_read(self.handle, C.byref(ms), C.byref(n)))
-        return float(ms.value), int(n.value)
+    def profile_read(self, kind: int, capacity: int = 1 << 16):
+        """Per-launch durations (ms, launch order) of one kernel kind since the last read."""
+        buf = (C.c_double * capacity)()
+        n = C.c_int32(0)
+        self._check(self.lib.slack_profile_read(self.handle, int(kind), buf, capacity, C.byref(n)))
+        return [float(buf[i]) for i in range(min(int(n.value), capacity))]
 
-    # --- diagnostics --------------------------------------------------------------------------------------------------
-    def debug_set_s_dump(self, tensor) -> None:
-        self._check(self.lib.slack_debug_set(self.handle, 0, _ptr(tensor)))
+    # --- diagnostics (library built with SLACK_DIAGNOSTICS=1 only; include/slack_diag.h) ------------------------------
+    def debug_set(self, key: int, tensor) -> None:
+        if not hasattr(self.lib, "slack_debug_set"):
+            raise RuntimeError("libslack.so was built without -DSLACK_DIAGNOSTICS")
+        self._check(self.lib.slack_debug_set(self.handle, int(key), _ptr(tensor)))
 
-    def debug_set_trace(self, tensor) -> None:
-        """int32 device tensor of 2048 + 4 * n_sm words (or None): clock trace, see include/slack.h."""
-        self._check(self.lib.slack_debug_set(self.handle, 1, _ptr(tensor)))
 
-    def debug_use_cluster_kernel(self, on: bool) -> None:
-        """Route dense tensor-core launches of plans made for <= sm_count / 2 queues to the 2-CTA-cluster kernel."""
-        self._check(self.lib.slack_debug_set(self.handle, 2, C.c_void_p(1) if on else None))
+class Cache:
+    """slack_cache_t wrapper: page bookkeeping of one pool shape (A0 / A5, host only).  begin_chunk returns a descriptor
+    object with the StreamSpec fields (page_table copied out as a numpy array)."""
 
-    def debug_timeout(self):
-        buf = (C.c_uint64 * 4)()
-        self.lib.slack_debug_timeout(self.handle, buf)
-        return [int(x) for x in buf]
+    class Desc:
+        def __init__(self, c: "CStream"):
+            self.q_len, self.cache_len, self.base, self.window = c.q_len, c.cache_len, c.base, c.window
+            self.sink_len, self.gap_slots = c.sink_len, c.gap_slots
+            self.page_table = np.ctypeslib.as_array(c.page_table, shape=(c.n_table_pages,)).copy() if c.n_table_pages else \
+                np.zeros(0, dtype=np.int32)
+
+        @property
+        def n(self) -> int:
+            return self.cache_len + self.q_len
+
+    def __init__(self, n_pages: int, page_size: int, trim_policy: int = TRIM_PAGES):
+        self.lib = load()
+        h = _VP()
+        st = self.lib.slack_cache_create(n_pages, page_size, trim_policy, C.byref(h))
+        if st != SLACK_OK:
+            raise SlackError(st, "slack_cache_create failed")
+        self.handle = h.value
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.slack_cache_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != SLACK_OK:
+            raise SlackError(st, self.lib.slack_cache_last_error(self.handle).decode())
+
+    def open(self, window: int = 0, sink_len: int = 0) -> int:
+        sid = C.c_int32(-1)
+        self._check(self.lib.slack_cache_open(self.handle, window, sink_len, C.byref(sid)))
+        return int(sid.value)
+
+    def begin_chunk(self, stream_id: int, q_len: int) -> "Cache.Desc":
+        c = CStream()
+        self._check(self.lib.slack_cache_begin_chunk(self.handle, stream_id, q_len, C.byref(c)))
+        return Cache.Desc(c)
+
+    def commit(self, stream_id: int) -> None:
+        self._check(self.lib.slack_cache_commit(self.handle, stream_id))
+
+    def close_stream(self, stream_id: int) -> None:
+        self._check(self.lib.slack_cache_close(self.handle, stream_id))
+
+    @property
+    def free_pages(self) -> int:
+        return int(self.lib.slack_cache_free_pages(self.handle))
+
+    def stream_pages(self, stream_id: int) -> int:
+        return int(self.lib.slack_cache_stream_pages(self.handle, stream_id))
 
 
 # ---------------------------------------------------------------------------------------------------------------------

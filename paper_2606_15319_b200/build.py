@@ -3,6 +3,8 @@
     python -m paper_2606_15319_b200.build [--force] [--verbose]
 
 nvcc cross-compiles without a GPU.  The library is rebuilt when any source or header is newer than the .so.
+SLACK_DIAGNOSTICS=1 in the environment builds the diagnostics flavour (include/slack_diag.h: S-tile dump and clock trace
+of the attention kernel); the default library carries neither the calls nor the traced kernel instantiation.
 """
 from __future__ import annotations
 
@@ -15,7 +17,7 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 INCLUDE = os.path.join(os.path.dirname(PKG_DIR), "include")
 LIB_PATH = os.path.join(PKG_DIR, "libslack.so")
-SOURCES = ["api.cu", "plan.cpp", "append.cu", "attn_simt.cu", "attn_tc.cu", "attn_tc2.cu", "combine.cu", "sparse_steps.cu", "transfer.cu"]
+SOURCES = ["api.cu", "plan.cpp", "pager.cpp", "append.cu", "attn_simt.cu", "attn_tc.cu", "combine.cu", "sparse_steps.cu", "transfer.cu"]
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
@@ -42,6 +44,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     build_dir = os.path.join(PKG_DIR, "build")
     os.makedirs(build_dir, exist_ok=True)
     common = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE] + ARCH_FLAGS
+    if os.environ.get("SLACK_DIAGNOSTICS", "0") not in ("", "0"):
+        common += ["-DSLACK_DIAGNOSTICS"]
     if verbose:
         common += ["-Xptxas", "-v"]
     procs = []

@@ -19,6 +19,140 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+namespace {
+
+// ---- ctx-owned arena: device memory + a pinned host mirror of the same size ---------------------------------------
+// Plan tables and the staging tables of slack_kv_append / slack_kv_transfer are cut out of it (first fit, coalescing
+// free list).  A block is filled through its host mirror and copied with one cudaMemcpyAsync; it is handed back by
+// release_after(events): the block returns to the free list once every event has completed, so nothing ever waits for
+// the device on the host (the staging buffer used to be re-used while kernels of an earlier call on another
+// stream were still reading it).  Segments are added when the arena runs dry (rare: a few MB hold hundreds of plans).
+struct ArenaBlock {
+  int seg = -1;
+  size_t off = 0, size = 0;
+  explicit operator bool() const { return seg >= 0; }
+};
+
+struct Arena {
+  struct Segment {
+    uint8_t *dev = nullptr, *host = nullptr;
+    size_t cap = 0;
+    std::vector<std::pair<size_t, size_t>> free_list; // (offset, size), sorted by offset, coalesced
+  };
+  struct Pending {
+    ArenaBlock blk;
+    std::vector<cudaEvent_t> events;
+  };
+  std::vector<Segment> segs;
+  std::vector<Pending> pending;
+  std::vector<cudaEvent_t> event_pool;
+
+  cudaError_t get_event(cudaEvent_t *ev) {
+    if (!event_pool.empty()) {
+      *ev = event_pool.back();
+      event_pool.pop_back();
+      return cudaSuccess;
+    }
+    return cudaEventCreateWithFlags(ev, cudaEventDisableTiming);
+  }
+  void put_event(cudaEvent_t ev) { event_pool.push_back(ev); }
+
+  void free_now(const ArenaBlock &b) {
+    auto &fl = segs[(size_t)b.seg].free_list;
+    auto it = std::lower_bound(fl.begin(), fl.end(), std::make_pair(b.off, (size_t)0));
+    it = fl.insert(it, {b.off, b.size});
+    if (it + 1 != fl.end() && it->first + it->second == (it + 1)->first) {
+      it->second += (it + 1)->second;
+      fl.erase(it + 1);
+    }
+    if (it != fl.begin() && (it - 1)->first + (it - 1)->second == it->first) {
+      (it - 1)->second += it->second;
+      fl.erase(it);
+    }
+  }
+  // blocks whose guarding events have all completed go back to the free lists (never blocks)
+  void reclaim() {
+    for (size_t i = 0; i < pending.size();) {
+      Pending &p = pending[i];
+      while (!p.events.empty() && cudaEventQuery(p.events.back()) == cudaSuccess) {
+        put_event(p.events.back());
+        p.events.pop_back();
+      }
+      if (p.events.empty()) {
+        free_now(p.blk);
+        pending[i] = std::move(pending.back());
+        pending.pop_back();
+      } else {
+        ++i;
+      }
+    }
+    (void)cudaGetLastError(); // cudaErrorNotReady from the queries is not an error
+  }
+  void release_after(const ArenaBlock &b, std::vector<cudaEvent_t> &&events) {
+    if (!b) return;
+    if (events.empty()) {
+      free_now(b);
+      return;
+    }
+    pending.push_back({b, std::move(events)});
+  }
+  ArenaBlock try_alloc(size_t size) {
+    for (size_t si = 0; si < segs.size(); ++si) {
+      auto &fl = segs[si].free_list;
+      for (size_t i = 0; i < fl.size(); ++i)
+        if (fl[i].second >= size) {
+          ArenaBlock b;
+          b.seg = (int)si;
+          b.off = fl[i].first;
+          b.size = size;
+          fl[i].first += size;
+          fl[i].second -= size;
+          if (fl[i].second == 0) fl.erase(fl.begin() + (long)i);
+          return b;
+        }
+    }
+    return ArenaBlock();
+  }
+  cudaError_t alloc(size_t size, ArenaBlock *out) {
+    size = (size + 255) & ~(size_t)255;
+    if (size == 0) size = 256;
+    reclaim();
+    *out = try_alloc(size);
+    if (*out) return cudaSuccess;
+    Segment sg;
+    sg.cap = std::max<size_t>(size * 2, segs.empty() ? ((size_t)4 << 20) : segs.back().cap * 2);
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&sg.dev), sg.cap);
+    if (e != cudaSuccess) return e;
+    e = cudaMallocHost(reinterpret_cast<void **>(&sg.host), sg.cap);
+    if (e != cudaSuccess) {
+      cudaFree(sg.dev);
+      return e;
+    }
+    sg.free_list.push_back({0, sg.cap});
+    segs.push_back(std::move(sg));
+    *out = try_alloc(size);
+    return *out ? cudaSuccess : cudaErrorMemoryAllocation;
+  }
+  uint8_t *dev(const ArenaBlock &b) const { return segs[(size_t)b.seg].dev + b.off; }
+  uint8_t *host(const ArenaBlock &b) const { return segs[(size_t)b.seg].host + b.off; }
+  void destroy() { // after a device synchronisation
+    for (Pending &p : pending)
+      for (cudaEvent_t e : p.events) cudaEventDestroy(e);
+    for (cudaEvent_t e : event_pool) cudaEventDestroy(e);
+    for (Segment &sg : segs) {
+      cudaFree(sg.dev);
+      cudaFreeHost(sg.host);
+    }
+    pending.clear();
+    event_pool.clear();
+    segs.clear();
+  }
+};
+
+constexpr int kProfKinds = 3; // bit index of SLACK_PROF_ATTENTION / _APPEND / _COMBINE
+
+} // namespace
+
 struct slack_ctx {
   int device = -1;
   int sm_count = 148;
@@ -26,43 +160,36 @@ struct slack_ctx {
   int last_launches = 0;
   EncodeTiledFn encode = nullptr;
   bool tc_configured = false;
-  // staging for slack_kv_append (descriptor tables of an unplanned append)
-  void *h_stage = nullptr;
-  void *d_stage = nullptr;
-  size_t stage_cap = 0;
-  cudaEvent_t stage_ev = nullptr;
-  bool stage_pending = false;
-  // staging for slack_kv_transfer (source / destination page id lists)
-  void *h_xfer = nullptr;
-  void *d_xfer = nullptr;
-  size_t xfer_cap = 0;
-  cudaEvent_t xfer_ev = nullptr;
-  bool xfer_pending = false;
+  Arena arena;
   // plan tables are uploaded on a private non-blocking stream: slack_plan never waits for the caller's queued work
   cudaStream_t up_stream = nullptr;
-  // diagnostics
-  unsigned long long *h_dbg = nullptr; // mapped pinned, 4 words, survives a trapped launch
+  std::vector<slack_plan_s *> live_plans; // orphaned (ctx = NULL) by slack_destroy
+  // time-out record of the in-kernel barrier waits: mapped pinned, 4 words, survives a trapped launch
+  unsigned long long *h_dbg = nullptr;
   unsigned long long *d_dbg = nullptr;
+#ifdef SLACK_DIAGNOSTICS
   float *dbg_s = nullptr;
   uint32_t *dbg_t = nullptr;
-  bool use_cluster_kernel = false; // debug key 2: the 2-CTA-cluster attention kernel (attn_tc2.cu) for dense plans
-  bool tc2_configured = false;
-  // per-launch timing of the attention kernel (slack_profile_attention)
-  bool prof_on = false;
-  std::vector<cudaEvent_t> prof_events; // pairs: [2i] before, [2i+1] after
-  size_t prof_used = 0;                 // pairs recorded since the last read
+#endif
+  // per-launch timing (slack_profile_enable): event pairs per kind, [2i] before, [2i+1] after
+  int prof_mask = 0;
+  std::vector<cudaEvent_t> prof_events[kProfKinds];
+  size_t prof_used[kProfKinds] = {0, 0, 0};
 };
 
 struct slack_plan_s {
-  slack_ctx *ctx = nullptr;
+  slack_ctx *ctx = nullptr; // NULL once the context is gone
   HostPlan hp;
   int max_q_len = 0;
-  void *d_blob = nullptr; // one allocation holding all tables
+  ArenaBlock blk;           // one arena block holding all tables
   DevStream *d_streams = nullptr;
   int32_t *d_page_tables = nullptr;
   DevItem *d_items = nullptr;
   int32_t *d_cta_begin = nullptr;
   DevCombine *d_combines = nullptr;
+  // bookkeeping of a plan in use (a plan's TABLES are immutable; this is not part of them)
+  mutable cudaEvent_t ready_ev = nullptr;      // upload finished; NULL once that has been observed
+  mutable std::vector<cudaStream_t> used_on;   // streams that ran kernels reading the tables
 };
 
 namespace {
@@ -72,8 +199,11 @@ slack_status set_err(slack_ctx *ctx, slack_status st, const std::string &msg) {
   return st;
 }
 slack_status cuda_err(slack_ctx *ctx, cudaError_t e, const char *what) {
-  char buf[256];
-  snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+  char buf[384];
+  int n = snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+  if (ctx && ctx->h_dbg && ctx->h_dbg[0] == 0xDEADull && n > 0 && (size_t)n < sizeof buf)
+    snprintf(buf + n, sizeof buf - (size_t)n, " [a bounded barrier wait timed out: block %llu thread %llu barrier tag %llu parity %llu]",
+             ctx->h_dbg[1] >> 32, ctx->h_dbg[1] & 0xffffffffull, ctx->h_dbg[2] >> 32, ctx->h_dbg[2] & 0xffffffffull);
   return set_err(ctx, SLACK_ECUDA, buf);
 }
 #define SLACK_CUDA(ctx, call)                                  \
@@ -121,6 +251,44 @@ slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t
 
 int elem_bytes(int dtype) { return dtype == SLACK_BF16 ? 2 : 4; }
 
+// The first launches that use a plan wait, on the device, for its upload; every stream that reads the tables is noted
+// so that slack_plan_destroy can guard the block with an event per stream.
+slack_status plan_in_use(slack_ctx *ctx, const slack_plan_s *plan, cudaStream_t cs) {
+  if (plan->ready_ev) {
+    if (cudaEventQuery(plan->ready_ev) == cudaSuccess) {
+      ctx->arena.put_event(plan->ready_ev);
+      plan->ready_ev = nullptr;
+    } else {
+      (void)cudaGetLastError();
+      SLACK_CUDA(ctx, cudaStreamWaitEvent(cs, plan->ready_ev, 0));
+    }
+  }
+  if (std::find(plan->used_on.begin(), plan->used_on.end(), cs) == plan->used_on.end()) plan->used_on.push_back(cs);
+  return SLACK_OK;
+}
+
+// event pair around one kernel launch (slack_profile_enable); returns the "after" event to record, or NULL
+slack_status prof_begin(slack_ctx *ctx, int kind_bit, cudaStream_t cs, cudaEvent_t *after) {
+  *after = nullptr;
+  if (!(ctx->prof_mask & (1 << kind_bit))) return SLACK_OK;
+  auto &ev = ctx->prof_events[kind_bit];
+  size_t &used = ctx->prof_used[kind_bit];
+  while (ev.size() < 2 * (used + 1)) {
+    cudaEvent_t e;
+    SLACK_CUDA(ctx, cudaEventCreate(&e));
+    ev.push_back(e);
+  }
+  SLACK_CUDA(ctx, cudaEventRecord(ev[2 * used], cs));
+  *after = ev[2 * used + 1];
+  return SLACK_OK;
+}
+slack_status prof_end(slack_ctx *ctx, int kind_bit, cudaStream_t cs, cudaEvent_t after) {
+  if (!after) return SLACK_OK;
+  SLACK_CUDA(ctx, cudaEventRecord(after, cs));
+  ctx->prof_used[kind_bit]++;
+  return SLACK_OK;
+}
+
 } // namespace
 
 extern "C" {
@@ -144,7 +312,6 @@ slack_status slack_create(slack_ctx **out, int device) {
       e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
       if (e == cudaSuccess && qres == cudaDriverEntryPointSuccess) ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
     }
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->stage_ev, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->up_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) {
       e = cudaHostAlloc(reinterpret_cast<void **>(&ctx->h_dbg), 4 * sizeof(unsigned long long), cudaHostAllocMapped);
@@ -164,19 +331,19 @@ slack_status slack_create(slack_ctx **out, int device) {
 
 void slack_destroy(slack_ctx *ctx) {
   if (!ctx) return;
+  for (slack_plan_s *pl : ctx->live_plans) { // plans may outlive the context: they keep their host tables only
+    pl->ctx = nullptr;
+    pl->blk = ArenaBlock();
+    pl->ready_ev = nullptr;
+  }
   if (ctx->device >= 0) {
     cudaSetDevice(ctx->device);
-    if (ctx->stage_pending) cudaEventSynchronize(ctx->stage_ev);
-    if (ctx->stage_ev) cudaEventDestroy(ctx->stage_ev);
+    cudaDeviceSynchronize(); // kernels that read arena blocks have finished
+    ctx->arena.destroy();
     if (ctx->up_stream) cudaStreamDestroy(ctx->up_stream);
-    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
-    if (ctx->d_stage) cudaFree(ctx->d_stage);
-    if (ctx->xfer_pending) cudaEventSynchronize(ctx->xfer_ev);
-    if (ctx->xfer_ev) cudaEventDestroy(ctx->xfer_ev);
-    if (ctx->h_xfer) cudaFreeHost(ctx->h_xfer);
-    if (ctx->d_xfer) cudaFree(ctx->d_xfer);
     if (ctx->h_dbg) cudaFreeHost(ctx->h_dbg);
-    for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
+    for (auto &v : ctx->prof_events)
+      for (cudaEvent_t e : v) cudaEventDestroy(e);
   }
   delete ctx;
 }
@@ -184,8 +351,8 @@ void slack_destroy(slack_ctx *ctx) {
 const char *slack_last_error(const slack_ctx *ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
 int32_t slack_last_launch_count(const slack_ctx *ctx) { return ctx ? ctx->last_launches : 0; }
 
-/* diagnostics (not part of the data path): key 0 = device pointer of a [2][128][128] fp32 buffer receiving the first
- * S tiles of CTA 0 (NULL disables); key 1 = device pointer of a [3][64][8] uint32 clock trace of CTA 0's first item; slack_debug_timeout copies the 4-word time-out record of the last trapped launch. */
+#ifdef SLACK_DIAGNOSTICS
+/* diagnostics build only (include/slack_diag.h) */
 slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value) {
   if (!ctx) return SLACK_EINVAL;
   if (key == 0) {
@@ -196,38 +363,36 @@ slack_status slack_debug_set(slack_ctx *ctx, int32_t key, void *value) {
     ctx->dbg_t = reinterpret_cast<uint32_t *>(value);
     return SLACK_OK;
   }
-  if (key == 2) {
-    ctx->use_cluster_kernel = value != nullptr;
-    return SLACK_OK;
-  }
   return set_err(ctx, SLACK_EINVAL, "unknown debug key");
 }
-slack_status slack_debug_timeout(slack_ctx *ctx, uint64_t out[4]) {
-  if (!ctx || !out) return SLACK_EINVAL;
-  for (int i = 0; i < 4; ++i) out[i] = ctx->h_dbg ? ctx->h_dbg[i] : 0;
-  return SLACK_OK;
-}
+#endif
 
-slack_status slack_profile_attention(slack_ctx *ctx, int32_t enable) {
+slack_status slack_profile_enable(slack_ctx *ctx, int32_t kinds) {
   if (!ctx) return SLACK_EINVAL;
-  ctx->prof_on = enable != 0;
+  if (kinds < 0 || kinds >= (1 << kProfKinds)) return set_err(ctx, SLACK_EINVAL, "unknown profile kind");
+  ctx->prof_mask = kinds;
   return SLACK_OK;
 }
-slack_status slack_profile_read(slack_ctx *ctx, double *total_ms, int32_t *n_launches) {
-  if (!ctx || !total_ms || !n_launches) return SLACK_EINVAL;
-  *total_ms = 0;
+slack_status slack_profile_read(slack_ctx *ctx, int32_t kind, double *ms_out, int32_t capacity, int32_t *n_launches) {
+  if (!ctx || !n_launches || capacity < 0 || (capacity > 0 && !ms_out)) return SLACK_EINVAL;
   *n_launches = 0;
-  if (ctx->prof_used == 0) return SLACK_OK;
+  int bit = -1;
+  for (int b = 0; b < kProfKinds; ++b)
+    if (kind == (1 << b)) bit = b;
+  if (bit < 0) return set_err(ctx, SLACK_EINVAL, "slack_profile_read: kind must be exactly one SLACK_PROF_* bit");
+  const size_t used = ctx->prof_used[bit];
+  if (used == 0) return SLACK_OK;
   slack_status st = ensure_device(ctx);
   if (st != SLACK_OK) return st;
-  for (size_t i = 0; i < ctx->prof_used; ++i) {
+  const auto &ev = ctx->prof_events[bit];
+  for (size_t i = 0; i < used; ++i) {
     float ms = 0.f;
-    SLACK_CUDA(ctx, cudaEventSynchronize(ctx->prof_events[2 * i + 1]));
-    SLACK_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->prof_events[2 * i], ctx->prof_events[2 * i + 1]));
-    *total_ms += ms;
+    SLACK_CUDA(ctx, cudaEventSynchronize(ev[2 * i + 1]));
+    SLACK_CUDA(ctx, cudaEventElapsedTime(&ms, ev[2 * i], ev[2 * i + 1]));
+    if ((int32_t)i < capacity) ms_out[i] = ms;
   }
-  *n_launches = (int32_t)ctx->prof_used;
-  ctx->prof_used = 0;
+  *n_launches = (int32_t)used;
+  ctx->prof_used[bit] = 0;
   return SLACK_OK;
 }
 
@@ -269,10 +434,16 @@ slack_status slack_plan(slack_ctx *ctx, const slack_pool *pool_shape, int32_t n_
     const size_t b_cta = align_up(hp.cta_begin.size() * sizeof(int32_t), 256);
     const size_t b_comb = align_up(hp.combines.size() * sizeof(DevCombine) + 16, 256);
     const size_t total = b_streams + b_pt + b_items + b_cta + b_comb;
-    std::vector<uint8_t> blob(total, 0);
+    cudaError_t e = ctx->arena.alloc(total, &pl->blk);
+    if (e != cudaSuccess) {
+      delete pl;
+      return cuda_err(ctx, e, "plan tables: arena allocation");
+    }
+    uint8_t *h = ctx->arena.host(pl->blk);
+    memset(h, 0, total);
     size_t off = 0;
     auto put = [&](const void *src, size_t n, size_t padded) {
-      if (n) memcpy(blob.data() + off, src, n);
+      if (n) memcpy(h + off, src, n);
       const size_t at = off;
       off += padded;
       return at;
@@ -282,30 +453,57 @@ slack_status slack_plan(slack_ctx *ctx, const slack_pool *pool_shape, int32_t n_
     const size_t o_items = put(hp.items.data(), hp.items.size() * sizeof(DevItem), b_items);
     const size_t o_cta = put(hp.cta_begin.data(), hp.cta_begin.size() * sizeof(int32_t), b_cta);
     const size_t o_comb = put(hp.combines.data(), hp.combines.size() * sizeof(DevCombine), b_comb);
-    cudaError_t e = cudaMalloc(&pl->d_blob, total);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_blob, blob.data(), total, cudaMemcpyHostToDevice, ctx->up_stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->up_stream); // the tables are resident when slack_plan returns
+    uint8_t *b = ctx->arena.dev(pl->blk);
+    // asynchronous upload from the pinned mirror; the first launches that use the plan wait for ready_ev on the device
+    e = cudaMemcpyAsync(b, h, total, cudaMemcpyHostToDevice, ctx->up_stream);
+    if (e == cudaSuccess) e = ctx->arena.get_event(&pl->ready_ev);
+    if (e == cudaSuccess) e = cudaEventRecord(pl->ready_ev, ctx->up_stream);
     if (e != cudaSuccess) {
-      if (pl->d_blob) cudaFree(pl->d_blob);
+      cudaStreamSynchronize(ctx->up_stream);
+      ctx->arena.free_now(pl->blk);
       delete pl;
       return cuda_err(ctx, e, "plan upload");
     }
-    uint8_t *b = reinterpret_cast<uint8_t *>(pl->d_blob);
     pl->d_streams = reinterpret_cast<DevStream *>(b + o_streams);
     pl->d_page_tables = reinterpret_cast<int32_t *>(b + o_pt);
     pl->d_items = reinterpret_cast<DevItem *>(b + o_items);
     pl->d_cta_begin = reinterpret_cast<int32_t *>(b + o_cta);
     pl->d_combines = reinterpret_cast<DevCombine *>(b + o_comb);
   }
+  ctx->live_plans.push_back(pl);
   *plan_out = pl;
   return SLACK_OK;
 }
 
 void slack_plan_destroy(slack_plan_t *plan) {
   if (!plan) return;
-  if (plan->d_blob) {
-    if (plan->ctx && plan->ctx->device >= 0) cudaSetDevice(plan->ctx->device);
-    cudaFree(plan->d_blob); // synchronises with outstanding work that may still read the tables
+  slack_ctx *ctx = plan->ctx;
+  if (ctx) {
+    auto it = std::find(ctx->live_plans.begin(), ctx->live_plans.end(), plan);
+    if (it != ctx->live_plans.end()) ctx->live_plans.erase(it);
+    if (plan->blk && ctx->device >= 0) {
+      int cur = -1;
+      if (cudaGetDevice(&cur) == cudaSuccess && cur != ctx->device) cudaSetDevice(ctx->device);
+      // the block returns to the arena once the upload and every stream that read the tables have passed this point
+      std::vector<cudaEvent_t> guard;
+      if (plan->ready_ev) guard.push_back(plan->ready_ev);
+      bool ok = true;
+      for (cudaStream_t cs : plan->used_on) {
+        cudaEvent_t ev;
+        if (ctx->arena.get_event(&ev) != cudaSuccess || cudaEventRecord(ev, cs) != cudaSuccess) {
+          ok = false;
+          break;
+        }
+        guard.push_back(ev);
+      }
+      if (!ok) { // cannot guard it: fall back to waiting for the device once
+        cudaDeviceSynchronize();
+        (void)cudaGetLastError();
+        for (cudaEvent_t ev : guard) ctx->arena.put_event(ev);
+        guard.clear();
+      }
+      ctx->arena.release_after(plan->blk, std::move(guard));
+    }
   }
   delete plan;
 }
@@ -349,16 +547,21 @@ slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, c
   if (!plan) return set_err(ctx, SLACK_EINVAL, "plan NULL");
   slack_status st = ensure_device(ctx);
   if (st != SLACK_OK) return st;
+  if (plan->ctx != ctx) return set_err(ctx, SLACK_EINVAL, "plan belongs to another context");
   st = check_pool(ctx, pool, &plan->hp);
   if (st != SLACK_OK) return st;
   if (plan->hp.total_q == 0) return SLACK_OK;
   if (!k_new || !v_new || !aligned(k_new, 16) || !aligned(v_new, 16))
     return set_err(ctx, SLACK_EINVAL, "k_new / v_new NULL or not 16-byte aligned");
   const HostPlan &hp = plan->hp;
+  cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
+  cudaEvent_t ev_after;
+  if ((st = prof_begin(ctx, 1, cs, &ev_after)) != SLACK_OK) return st;
   SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, plan->d_streams, hp.n_streams, plan->max_q_len,
                                    plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, elem_bytes(hp.dtype),
-                                   ctx->sm_count, reinterpret_cast<cudaStream_t>(cuda_stream), &ctx->last_launches));
-  return SLACK_OK;
+                                   ctx->sm_count, cs, &ctx->last_launches));
+  return prof_end(ctx, 1, cs, ev_after);
 }
 
 slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_streams, const slack_stream *streams,
@@ -387,32 +590,32 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
   const size_t b_pt = align_up(hp.page_tables.size() * sizeof(int32_t), 256);
   const size_t total = b_streams + b_pt;
   cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
-  if (ctx->stage_pending) { // the previous append's copy must have consumed the staging buffer
-    SLACK_CUDA(ctx, cudaEventSynchronize(ctx->stage_ev));
-    ctx->stage_pending = false;
-  }
-  if (total > ctx->stage_cap) {
-    if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
-    if (ctx->d_stage) cudaFree(ctx->d_stage); // device-synchronising: earlier appends have finished with it
-    ctx->h_stage = ctx->d_stage = nullptr;
-    ctx->stage_cap = 0;
-    const size_t cap = align_up(total * 2, 4096);
-    SLACK_CUDA(ctx, cudaMallocHost(&ctx->h_stage, cap));
-    SLACK_CUDA(ctx, cudaMalloc(&ctx->d_stage, cap));
-    ctx->stage_cap = cap;
-  }
-  uint8_t *h = reinterpret_cast<uint8_t *>(ctx->h_stage);
+  // descriptor tables: one arena block per call, filled through its pinned mirror, released by an event recorded
+  // BEHIND the kernel that reads it (two appends on different streams never share a staging buffer)
+  ArenaBlock blk;
+  SLACK_CUDA(ctx, ctx->arena.alloc(total, &blk));
+  uint8_t *h = ctx->arena.host(blk);
+  uint8_t *d = ctx->arena.dev(blk);
   memcpy(h, hp.streams.data(), hp.streams.size() * sizeof(DevStream));
   memcpy(h + b_streams, hp.page_tables.data(), hp.page_tables.size() * sizeof(int32_t));
-  SLACK_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage, h, total, cudaMemcpyHostToDevice, cs));
-  SLACK_CUDA(ctx, cudaEventRecord(ctx->stage_ev, cs));
-  ctx->stage_pending = true;
   int max_q = 0;
   for (const DevStream &s : hp.streams) max_q = s.q_len > max_q ? s.q_len : max_q;
-  uint8_t *d = reinterpret_cast<uint8_t *>(ctx->d_stage);
-  SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, reinterpret_cast<DevStream *>(d), hp.n_streams,
-                                   max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.head_dim, hp.page_size,
-                                   elem_bytes(hp.dtype), ctx->sm_count, cs, &ctx->last_launches));
+  cudaError_t e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, cs);
+  if (e == cudaSuccess)
+    e = launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, reinterpret_cast<DevStream *>(d), hp.n_streams, max_q,
+                         reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.head_dim, hp.page_size,
+                         elem_bytes(hp.dtype), ctx->sm_count, cs, &ctx->last_launches);
+  cudaEvent_t done = nullptr;
+  cudaError_t e2 = ctx->arena.get_event(&done);
+  if (e2 == cudaSuccess) e2 = cudaEventRecord(done, cs);
+  if (e2 != cudaSuccess) { // cannot guard the block: wait for the stream once, then free it
+    cudaStreamSynchronize(cs);
+    if (done) ctx->arena.put_event(done);
+    ctx->arena.free_now(blk);
+  } else {
+    ctx->arena.release_after(blk, std::vector<cudaEvent_t>{done});
+  }
+  if (e != cudaSuccess) return cuda_err(ctx, e, "slack_kv_append");
   return SLACK_OK;
 }
 
@@ -435,6 +638,7 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
     return set_err(ctx, SLACK_EUNSUPPORTED, "a (page, head) slice must be a multiple of 16 bytes");
   if (head_begin < 0 || head_end > s0.n_heads || head_begin >= head_end)
     return set_err(ctx, SLACK_EINVAL, "head range must satisfy 0 <= head_begin < head_end <= n_heads");
+  bool same_pool = false; // some layer copies inside one pool: a page may then not be both source and destination
   for (int32_t l = 0; l < n_layers; ++l) {
     const slack_pool &a = src_pools[l];
     const slack_pool &b = dst_pools[l];
@@ -443,6 +647,7 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
         a.n_pages != s0.n_pages || b.n_heads != s0.n_heads || b.head_dim != s0.head_dim || b.page_size != s0.page_size ||
         b.dtype != s0.dtype || b.n_pages != d0.n_pages)
       return set_err(ctx, SLACK_EINVAL, "all layers' pools must share one shape per side, and both sides H, D, P and dtype");
+    same_pool |= a.k_pool == b.k_pool || a.v_pool == b.v_pool || a.k_pool == b.v_pool || a.v_pool == b.k_pool;
   }
   {
     std::vector<uint8_t> seen((size_t)std::max(d0.n_pages, 0), 0);
@@ -452,40 +657,40 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
       if (seen[dst_page_ids[i]]) return set_err(ctx, SLACK_EINVAL, "destination page listed twice");
       seen[dst_page_ids[i]] = 1;
     }
+    if (same_pool)
+      for (int32_t i = 0; i < n_pages; ++i)
+        if (src_page_ids[i] < d0.n_pages && seen[src_page_ids[i]])
+          return set_err(ctx, SLACK_EINVAL, "source and destination are the same pool and a page is both read and written");
   }
   cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
   const size_t half = align_up((size_t)n_pages * sizeof(int32_t), 256);
   const size_t total = 2 * half;
-  if (ctx->xfer_pending) { // the previous transfer's upload must have consumed the staging buffer
-    SLACK_CUDA(ctx, cudaEventSynchronize(ctx->xfer_ev));
-    ctx->xfer_pending = false;
-  }
-  if (!ctx->xfer_ev) SLACK_CUDA(ctx, cudaEventCreateWithFlags(&ctx->xfer_ev, cudaEventDisableTiming));
-  if (total > ctx->xfer_cap) {
-    if (ctx->h_xfer) cudaFreeHost(ctx->h_xfer);
-    if (ctx->d_xfer) cudaFree(ctx->d_xfer); // device-synchronising: earlier transfers have finished with it
-    ctx->h_xfer = ctx->d_xfer = nullptr;
-    ctx->xfer_cap = 0;
-    const size_t cap = align_up(total * 2, 4096);
-    SLACK_CUDA(ctx, cudaMallocHost(&ctx->h_xfer, cap));
-    SLACK_CUDA(ctx, cudaMalloc(&ctx->d_xfer, cap));
-    ctx->xfer_cap = cap;
-  }
-  uint8_t *h = reinterpret_cast<uint8_t *>(ctx->h_xfer);
+  ArenaBlock blk; // id lists: released by an event behind the LAST layer's kernel
+  SLACK_CUDA(ctx, ctx->arena.alloc(total, &blk));
+  uint8_t *h = ctx->arena.host(blk);
   memcpy(h, src_page_ids, (size_t)n_pages * sizeof(int32_t));
   memcpy(h + half, dst_page_ids, (size_t)n_pages * sizeof(int32_t));
-  SLACK_CUDA(ctx, cudaMemcpyAsync(ctx->d_xfer, h, total, cudaMemcpyHostToDevice, cs));
-  SLACK_CUDA(ctx, cudaEventRecord(ctx->xfer_ev, cs));
-  ctx->xfer_pending = true;
-  const int32_t *d_src = reinterpret_cast<const int32_t *>(ctx->d_xfer);
-  const int32_t *d_dst = reinterpret_cast<const int32_t *>(reinterpret_cast<uint8_t *>(ctx->d_xfer) + half);
-  for (int32_t l = 0; l < n_layers; ++l) { // layer-major: layer l is complete when event l fires
-    SLACK_CUDA(ctx, launch_kv_transfer(src_pools[l].k_pool, src_pools[l].v_pool, dst_pools[l].k_pool, dst_pools[l].v_pool,
-                                       d_src, d_dst, n_pages, s0.n_heads, s0.head_dim, s0.page_size, elem_bytes(s0.dtype),
-                                       head_begin, head_end, ctx->sm_count, cs, &ctx->last_launches));
-    if (layer_done_events && layer_done_events[l])
-      SLACK_CUDA(ctx, cudaEventRecord(reinterpret_cast<cudaEvent_t>(layer_done_events[l]), cs));
+  const int32_t *d_src = reinterpret_cast<const int32_t *>(ctx->arena.dev(blk));
+  const int32_t *d_dst = reinterpret_cast<const int32_t *>(ctx->arena.dev(blk) + half);
+  cudaError_t e = cudaMemcpyAsync(ctx->arena.dev(blk), h, total, cudaMemcpyHostToDevice, cs);
+  for (int32_t l = 0; l < n_layers && e == cudaSuccess; ++l) { // layer-major: layer l is complete when event l fires
+    e = launch_kv_transfer(src_pools[l].k_pool, src_pools[l].v_pool, dst_pools[l].k_pool, dst_pools[l].v_pool, d_src, d_dst,
+                           n_pages, s0.n_heads, s0.head_dim, s0.page_size, elem_bytes(s0.dtype), head_begin, head_end,
+                           ctx->sm_count, cs, &ctx->last_launches);
+    if (e == cudaSuccess && layer_done_events && layer_done_events[l])
+      e = cudaEventRecord(reinterpret_cast<cudaEvent_t>(layer_done_events[l]), cs);
   }
+  cudaEvent_t done = nullptr;
+  cudaError_t e2 = ctx->arena.get_event(&done);
+  if (e2 == cudaSuccess) e2 = cudaEventRecord(done, cs);
+  if (e2 != cudaSuccess) {
+    cudaStreamSynchronize(cs);
+    if (done) ctx->arena.put_event(done);
+    ctx->arena.free_now(blk);
+  } else {
+    ctx->arena.release_after(blk, std::vector<cudaEvent_t>{done});
+  }
+  if (e != cudaSuccess) return cuda_err(ctx, e, "slack_kv_transfer");
   return SLACK_OK;
 }
 
@@ -502,6 +707,7 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   if (!plan) return set_err(ctx, SLACK_EINVAL, "plan NULL");
   slack_status st = ensure_device(ctx);
   if (st != SLACK_OK) return st;
+  if (plan->ctx != ctx) return set_err(ctx, SLACK_EINVAL, "plan belongs to another context");
   st = check_pool(ctx, pool, &plan->hp);
   if (st != SLACK_OK) return st;
   const HostPlan &hp = plan->hp;
@@ -517,6 +723,7 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   }
 
   if (hp.kernel_kind == 1) {
+    if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
     SLACK_CUDA(ctx, launch_attn_simt(hp.dtype, q, pool->k_pool, pool->v_pool, out, lse, plan->d_streams, hp.n_streams, hp.total_q,
                                      plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, scale, block_mask, mask_words,
                                      cs, &ctx->last_launches));
@@ -540,14 +747,9 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   CUtensorMap tm_q, tm_k, tm_v;
   const uint64_t pool_rows = (uint64_t)hp.n_pages * hp.n_heads * hp.page_size;
   if ((st = make_map(ctx, &tm_q, q, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
-  const bool cluster2 = ctx->use_cluster_kernel && !block_mask && 2 * hp.n_cta <= ctx->sm_count;
-  const uint32_t kv_box_rows = cluster2 ? 64 : 128; // the cluster kernel loads half a key tile per CTA
-  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows, kv_box_rows)) != SLACK_OK) return st;
-  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows, kv_box_rows)) != SLACK_OK) return st;
-  if (cluster2 && !ctx->tc2_configured) {
-    SLACK_CUDA(ctx, attn_tc2_configure());
-    ctx->tc2_configured = true;
-  }
+  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
   TcParams p{};
   p.items = plan->d_items;
   p.cta_begin = plan->d_cta_begin;
@@ -556,8 +758,10 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   p.lse = lse;
   p.ws_o = reinterpret_cast<float *>(workspace);
   p.ws_lse = workspace ? reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + hp.ws.lse_off) : nullptr;
+#ifdef SLACK_DIAGNOSTICS
   p.dbg_s = ctx->dbg_s;
   p.dbg_t = ctx->dbg_t;
+#endif
   p.dbg_flag = ctx->d_dbg;
   p.n_heads = hp.n_heads;
   int pl2 = 0;
@@ -575,26 +779,16 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
     p.item_steps = item_steps;
     p.dbg_t = nullptr; // the clock-trace instantiation is dense-only
   }
-  cudaEvent_t ev_after = nullptr;
-  if (ctx->prof_on) {
-    while (ctx->prof_events.size() < 2 * (ctx->prof_used + 1)) {
-      cudaEvent_t e;
-      SLACK_CUDA(ctx, cudaEventCreate(&e));
-      ctx->prof_events.push_back(e);
-    }
-    SLACK_CUDA(ctx, cudaEventRecord(ctx->prof_events[2 * ctx->prof_used], cs));
-    ev_after = ctx->prof_events[2 * ctx->prof_used + 1];
+  cudaEvent_t ev_after;
+  if ((st = prof_begin(ctx, 0, cs, &ev_after)) != SLACK_OK) return st;
+  SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
+  if ((st = prof_end(ctx, 0, cs, ev_after)) != SLACK_OK) return st;
+  if (!hp.combines.empty()) {
+    if ((st = prof_begin(ctx, 2, cs, &ev_after)) != SLACK_OK) return st;
+    SLACK_CUDA(ctx, launch_combine(plan->d_combines, (int)hp.combines.size(), p.ws_o, p.ws_lse, out, lse, hp.n_heads, hp.head_dim,
+                                   hp.total_q, cs, &ctx->last_launches));
+    if ((st = prof_end(ctx, 2, cs, ev_after)) != SLACK_OK) return st;
   }
-  if (cluster2)
-    SLACK_CUDA(ctx, launch_attn_tc2(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
-  else
-    SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
-  if (ev_after) {
-    SLACK_CUDA(ctx, cudaEventRecord(ev_after, cs));
-    ctx->prof_used++;
-  }
-  SLACK_CUDA(ctx, launch_combine(plan->d_combines, (int)hp.combines.size(), p.ws_o, p.ws_lse, out, lse, hp.n_heads, hp.head_dim,
-                                 hp.total_q, cs, &ctx->last_launches));
   return SLACK_OK;
 }
 } // namespace

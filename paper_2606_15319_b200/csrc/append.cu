@@ -40,7 +40,7 @@ kv_append_kernel(const uint4 *__restrict__ k_new, const uint4 *__restrict__ v_ne
         const int rem = (int)(u - (long long)tok * row_units);
         const int h = rem >> vec_log2;
         const int c = rem & (vecs - 1);
-        const int pos = s.base + s.cache_len + tok;
+        const int pos = s.app_pos0 + tok;
         const long long page = pt[pos >> page_log2];
         const int slot = pos & page_mask;
         dst[j] = ((((page * n_heads + h) << page_log2) + slot) << vec_log2) + c;
@@ -75,11 +75,15 @@ cudaError_t launch_kv_append(const void *k_new, const void *v_new, void *k_pool,
   long long cap = ((long long)sm_count * 8 + n_streams - 1) / n_streams;
   if (cap < 1) cap = 1;
   const int gx = (int)(want < cap ? want : cap);
-  dim3 grid(gx > 0 ? gx : 1, n_streams);
-  cudaError_t e = launch_pdl(kv_append_kernel, grid, dim3(kAppendThreads), 0, st, reinterpret_cast<const uint4 *>(k_new),
-                             reinterpret_cast<const uint4 *>(v_new), reinterpret_cast<uint4 *>(k_pool),
-                             reinterpret_cast<uint4 *>(v_pool), d_streams, d_page_tables, n_heads, ilog2(page_size), ilog2(vecs));
-  if (n_launched) *n_launched += 1;
+  constexpr int kMaxGridY = 65535; // gridDim.y limit: larger batches go out in several launches (same stream, in order)
+  cudaError_t e = cudaSuccess;
+  for (int s0 = 0; s0 < n_streams && e == cudaSuccess; s0 += kMaxGridY) {
+    const int ns = n_streams - s0 < kMaxGridY ? n_streams - s0 : kMaxGridY;
+    e = launch_pdl(kv_append_kernel, dim3(gx > 0 ? gx : 1, ns), dim3(kAppendThreads), 0, st, reinterpret_cast<const uint4 *>(k_new),
+                   reinterpret_cast<const uint4 *>(v_new), reinterpret_cast<uint4 *>(k_pool), reinterpret_cast<uint4 *>(v_pool),
+                   d_streams + s0, d_page_tables, n_heads, ilog2(page_size), ilog2(vecs));
+    if (n_launched) *n_launched += 1;
+  }
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 

@@ -110,11 +110,11 @@ __device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
 
 } // namespace
 
-// kTrace: diagnostic build that records clock64() time stamps of CTA 0's first item into p.dbg_t (slack_debug_set key 1):
+// kTrace (instantiated in -DSLACK_DIAGNOSTICS builds only): records clock64() time stamps of CTA 0's first item into p.dbg_t (slack_debug_set key 1):
 // [role 0/1 = softmax tile 0/1, 2 = MMA issuer, 3 = per-warp arrivals][kv step < 64][8 slots], then per-CTA spans.  The production instantiation has no trace code.
 #define SLACK_TRACE(role, step, slot)                                                                      \
   if constexpr (kTrace) {                                                                                  \
-    if (blockIdx.x == 0 && k == item_begin && (step) < 64 && (threadIdx.x & ((role) == 2 ? 31 : 127)) == 0)                    \
+    if (p.dbg_t != nullptr && blockIdx.x == 0 && k == item_begin && (step) < 64 && (threadIdx.x & ((role) == 2 ? 31 : 127)) == 0)                    \
       p.dbg_t[((role) * 64 + (step)) * 8 + (slot)] = (uint32_t)clock64();                                  \
   }
 
@@ -174,7 +174,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
   const int H = p.n_heads;
   const int P = 1 << p.page_log2;
   if constexpr (kTrace) { // per-CTA span: words [2048 + 4*cta .. +3] = {clock start, clock end, globaltimer start, end}
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && p.dbg_t != nullptr) {
       unsigned long long gt;
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
       p.dbg_t[2048 + 4 * blockIdx.x + 0] = (uint32_t)clock64();
@@ -415,9 +415,11 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 #pragma unroll
           for (int e = 0; e < 128; ++e) s[e] = (e >= c_lo && e < c_hi) ? s[e] : -INFINITY;
         }
-        if (p.dbg_s != nullptr && blockIdx.x == 0 && first_item && j == 0) {
+        if constexpr (kTrace) {
+          if (p.dbg_s != nullptr && blockIdx.x == 0 && first_item && j == 0) {
 #pragma unroll
-          for (int e = 0; e < 128; ++e) p.dbg_s[(i * 128 + row) * 128 + e] = s[e];
+            for (int e = 0; e < 128; ++e) p.dbg_s[(i * 128 + row) * 128 + e] = s[e];
+          }
         }
         // Row max of the tile: four independent FMNMX3 chains.  On the first tile of an item it is needed before any
         // exponential; later it is evaluated in the same instruction stream as the first 64 columns' exponentials
@@ -506,7 +508,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         if (lane == 0) mbar_arrive(bar(BAR_P_READY + i));
         SLACK_TRACE(i, j, 6);
         if constexpr (kTrace) { // per-warp arrival times (rows 3.. : [3][j][warp - 4])
-          if (blockIdx.x == 0 && k == item_begin && j < 64 && lane == 0) p.dbg_t[(3 * 64 + j) * 8 + (warp - 4)] = (uint32_t)clock64();
+          if (p.dbg_t != nullptr && blockIdx.x == 0 && k == item_begin && j < 64 && lane == 0) p.dbg_t[(3 * 64 + j) * 8 + (warp - 4)] = (uint32_t)clock64();
         }
         ++cnt;
       }
@@ -571,7 +573,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
   tc_fence_before();
   __syncthreads();
   if constexpr (kTrace) {
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && p.dbg_t != nullptr) {
       unsigned long long gt;
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
       p.dbg_t[2048 + 4 * blockIdx.x + 1] = (uint32_t)clock64();
@@ -590,8 +592,11 @@ cudaError_t attn_tc_configure() {
   cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+#ifdef SLACK_DIAGNOSTICS
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(attn_tc_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  e = cudaFuncSetAttribute(attn_tc_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+#endif
+  return e;
 }
 
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
@@ -599,8 +604,10 @@ cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUt
   cudaError_t e;
   if (p.steps != nullptr)
     e = launch_pdl(attn_tc_kernel<false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
-  else if (p.dbg_t != nullptr)
+#ifdef SLACK_DIAGNOSTICS
+  else if (p.dbg_t != nullptr || p.dbg_s != nullptr)
     e = launch_pdl(attn_tc_kernel<true, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+#endif
   else
     e = launch_pdl(attn_tc_kernel<false, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   if (n_launched) *n_launched += 1;

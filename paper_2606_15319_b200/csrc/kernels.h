@@ -55,9 +55,9 @@ struct TcParams {
   float *lse;           // [H][total_q] or null
   float *ws_o;          // partial outputs [slot][256][128] fp32
   float *ws_lse;        // partial lse [slot][256]
-  float *dbg_s;         // optional debug dump of the first S tiles of CTA 0 ([2][128][128] fp32), else null
-  uint32_t *dbg_t;      // optional time-stamp trace [3][64][8] (selects the kTrace instantiation), else null
-  unsigned long long *dbg_flag; // optional 4-word device buffer for time-out diagnostics, else null
+  float *dbg_s;         // SLACK_DIAGNOSTICS builds: dump of the first S tiles of CTA 0 ([2][128][128] fp32), else null
+  uint32_t *dbg_t;      // SLACK_DIAGNOSTICS builds: time-stamp trace (selects the kTrace instantiation), else null
+  unsigned long long *dbg_flag; // 4-word host-mapped record a timed-out barrier wait fills before it traps
   const uint16_t *steps;        // block-sparse: compacted step lists (sparse_steps.cu), else null = dense
   const int32_t *item_steps;    // block-sparse: selected steps per item
   int32_t n_heads;
@@ -69,12 +69,6 @@ size_t attn_tc_smem_bytes();
 cudaError_t attn_tc_configure(); // cudaFuncSetAttribute(max dynamic smem); once per process/device
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched);
-
-// A3 on 2-CTA clusters (attn_tc2.cu): one query tile per SM, K/V tiles multicast; `n_clusters` = the plan's queues.
-size_t attn_tc2_smem_bytes();
-cudaError_t attn_tc2_configure();
-cudaError_t launch_attn_tc2(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
-                            int n_clusters, cudaStream_t st, int *n_launched);
 
 // Block-sparse A3: per item, the selected key-tile steps under a device block mask (see sparse_steps.cu).
 cudaError_t launch_sparse_steps(const DevItem *d_items, int n_items, const uint32_t *mask, int n_heads, int mask_words,

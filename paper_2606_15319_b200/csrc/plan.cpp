@@ -290,14 +290,19 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
       snprintf(buf, sizeof buf, "stream %d: base %d outside [0, page_size)", i, s.base);
       return fail(SLACK_EINVAL, buf);
     }
-    if (s.sink_len < 0) {
-      snprintf(buf, sizeof buf, "stream %d: negative sink_len", i);
+    if (s.sink_len < 0 || s.gap_slots < 0) {
+      snprintf(buf, sizeof buf, "stream %d: negative sink_len / gap_slots", i);
+      return fail(SLACK_EINVAL, buf);
+    }
+    if (s.gap_slots > 0 && (s.sink_len == 0 || s.cache_len < s.sink_len)) {
+      snprintf(buf, sizeof buf, "stream %d: gap_slots needs sink_len > 0 and cache_len >= sink_len", i);
       return fail(SLACK_EINVAL, buf);
     }
     const int64_t n = (int64_t)s.cache_len + s.q_len;
-    if ((int64_t)s.base + n > (int64_t)INT32_MAX / 2 || row + s.q_len > (int64_t)INT32_MAX / 2)
+    const int64_t end_pos = (int64_t)s.base + s.gap_slots + n; // one past the position of token n - 1
+    if (end_pos > (int64_t)INT32_MAX / 2 || row + s.q_len > (int64_t)INT32_MAX / 2)
       return fail(SLACK_EINVAL, "batch too large for 32-bit token positions");
-    const int32_t need = n > 0 ? ceil_div((int64_t)s.base + n, P) : 0;
+    const int32_t need = n > 0 ? ceil_div(end_pos, P) : 0;
     if (s.n_table_pages < need) {
       snprintf(buf, sizeof buf, "stream %d: page table has %d pages, needs %d", i, s.n_table_pages, need);
       return fail(SLACK_EINVAL, buf);
@@ -310,17 +315,21 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     d.q_row0 = (int32_t)row;
     d.qblock0 = out.mask_rows;
     out.mask_rows += ceil_div(s.q_len, kItemRows);
-    out.mask_words_min = std::max<int32_t>(out.mask_words_min, ceil_div(ceil_div((int64_t)s.base + n, kTileN), 32));
+    out.mask_words_min = std::max<int32_t>(out.mask_words_min, ceil_div(ceil_div(end_pos, kTileN), 32));
     d.q_len = s.q_len;
     d.cache_len = s.cache_len;
     d.base = s.base;
-    // visible tokens = [0, sink) U [max(sink, lo), n) ("sink + local"); one range when they touch or overlap
+    // visible tokens = [0, sink) U [max(sink, lo), n) ("sink + local"); token t sits at position base + t, plus
+    // gap_slots behind the sink (slack.h).  One position range when the two touch and no slot is skipped between them.
     int64_t lo = (s.window > 0) ? std::max<int64_t>(0, n - s.window) : 0;
     const int64_t sink = std::min<int64_t>(s.sink_len, n);
-    if (lo <= sink) lo = 0;
-    d.pos_lo = (int32_t)(s.base + lo);
-    d.pos_hi = (int32_t)(s.base + n);
-    d.sink_hi = (int32_t)(s.base + (lo > 0 ? sink : 0));
+    const bool one_range = lo <= sink && s.gap_slots == 0;
+    if (one_range) lo = 0;
+    else lo = std::max(lo, sink);
+    d.pos_lo = (int32_t)(s.base + (one_range ? 0 : s.gap_slots) + lo);
+    d.pos_hi = (int32_t)end_pos;
+    d.sink_hi = (int32_t)(s.base + (one_range ? 0 : sink));
+    d.app_pos0 = (int32_t)(s.base + s.cache_len + (s.cache_len >= s.sink_len ? s.gap_slots : 0));
     d.pt_off = (int32_t)out.page_tables.size();
     d.n_table_pages = need;
     for (int32_t p = 0; p < need; ++p) {

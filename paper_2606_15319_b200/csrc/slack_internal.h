@@ -62,8 +62,10 @@ struct DevStream {
   int32_t n_table_pages;
   int32_t sink_hi;  // visible sink positions [base, sink_hi) in front of [pos_lo, pos_hi); == base when there are none
   int32_t qblock0;  // global index of the stream's first 256-row query block (row of the block mask)
+  int32_t app_pos0; // position of the first token the append writes: pos(cache_len) (slack.h token -> slot rule)
+  int32_t pad;
 };
-static_assert(sizeof(DevStream) == 40, "DevStream layout");
+static_assert(sizeof(DevStream) == 48, "DevStream layout");
 
 // Workspace layout for split-KV partials: slot s holds kItemRows rows of head_dim fp32 (normalised partial output)
 // followed, in a second region, by kItemRows fp32 lse values.

@@ -61,10 +61,14 @@ cudaError_t launch_kv_transfer(const void *src_k, const void *src_v, void *dst_k
   long long cap = ((long long)sm_count * 8 + n_pages - 1) / n_pages; // ~8 CTAs per SM over the whole grid
   if (cap < 1) cap = 1;
   const int gx = (int)(want < cap ? want : cap);
-  kv_transfer_kernel<<<dim3(gx > 0 ? gx : 1, n_pages), kXferThreads, 0, st>>>(
-      reinterpret_cast<const uint4 *>(src_k), reinterpret_cast<const uint4 *>(src_v), reinterpret_cast<uint4 *>(dst_k),
-      reinterpret_cast<uint4 *>(dst_v), d_src_ids, d_dst_ids, head_vecs * n_heads, head_vecs * head_begin, slice_vecs);
-  if (n_launched) *n_launched += 1;
+  constexpr int kMaxGridY = 65535; // gridDim.y limit: longer page lists go out in several launches (same stream, in order)
+  for (int p0 = 0; p0 < n_pages; p0 += kMaxGridY) {
+    const int np = n_pages - p0 < kMaxGridY ? n_pages - p0 : kMaxGridY;
+    kv_transfer_kernel<<<dim3(gx > 0 ? gx : 1, np), kXferThreads, 0, st>>>(
+        reinterpret_cast<const uint4 *>(src_k), reinterpret_cast<const uint4 *>(src_v), reinterpret_cast<uint4 *>(dst_k),
+        reinterpret_cast<uint4 *>(dst_v), d_src_ids + p0, d_dst_ids + p0, head_vecs * n_heads, head_vecs * head_begin, slice_vecs);
+    if (n_launched) *n_launched += 1;
+  }
   return cudaGetLastError();
 }
 

@@ -9,14 +9,8 @@ from typing import List
 
 def visible_keys(streams) -> List[int]:
     """Lk per stream: keys in [lo, n) plus the sink prefix, lo = max(0, n - Wt) when Wt > 0."""
-    out = []
-    for s in streams:
-        n = s.cache_len + s.q_len
-        lo = max(0, n - s.window) if s.window > 0 else 0
-        sink = min(s.sink_len, n)
-        lo = max(lo, sink)
-        out.append(n - lo + sink)
-    return out
+    from .workloads import visible_positions   # the one bookkeeping copy of the window formula outside oracle/ and csrc/
+    return [int(visible_positions(s).size) for s in streams]
 
 
 def attention_flops(streams, n_heads: int, head_dim: int) -> float:

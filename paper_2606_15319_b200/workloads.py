@@ -53,6 +53,7 @@ class StreamSpec:
     window: int                # Wt: max visible keys including the own chunk; 0 = unlimited
     sink_len: int              # leading tokens always visible ("sink + local"); 0 in all configs
     page_table: np.ndarray     # int32 [n_table_pages], logical page -> physical page
+    gap_slots: int = 0         # unused slots between the sink and the first held token behind it (include/slack.h)
 
     @property
     def n(self) -> int:
@@ -95,6 +96,7 @@ def _draw(rng: np.random.Generator, shape, amp: float, dtype: str) -> np.ndarray
 def make_workload(name: str, *, dtype: str, n_heads: int, head_dim: int, page_size: int,
                   q_lens: Sequence[int], cache_lens: Sequence[int], windows: Sequence[int],
                   bases: Optional[Sequence[int]] = None, sink_lens: Optional[Sequence[int]] = None,
+                  gap_slots: Optional[Sequence[int]] = None,
                   seed: int = 0, amp: float = 1.0, shuffle_pages: bool = True,
                   spare_pages: int = 0, scale: Optional[float] = None,
                   n_pages: Optional[int] = None) -> Workload:
@@ -107,7 +109,8 @@ def make_workload(name: str, *, dtype: str, n_heads: int, head_dim: int, page_si
     n_streams = len(q_lens)
     bases = list(bases) if bases is not None else [0] * n_streams
     sink_lens = list(sink_lens) if sink_lens is not None else [0] * n_streams
-    need = [-(-(bases[i] + cache_lens[i] + q_lens[i]) // page_size) for i in range(n_streams)]
+    gaps = list(gap_slots) if gap_slots is not None else [0] * n_streams
+    need = [-(-(bases[i] + gaps[i] + cache_lens[i] + q_lens[i]) // page_size) for i in range(n_streams)]
     total = int(sum(need)) + int(spare_pages)
     if n_pages is None:
         n_pages = max(total, 1)
@@ -121,7 +124,7 @@ def make_workload(name: str, *, dtype: str, n_heads: int, head_dim: int, page_si
         table = np.ascontiguousarray(order[at:at + need[i]], dtype=np.int32)
         at += need[i]
         streams.append(StreamSpec(int(q_lens[i]), int(cache_lens[i]), int(bases[i]), int(windows[i]),
-                                  int(sink_lens[i]), table))
+                                  int(sink_lens[i]), table, int(gaps[i])))
     tq = int(sum(q_lens))
     q = _draw(rng, (tq, n_heads, head_dim), amp, dtype)
     k_new = _draw(rng, (tq, n_heads, head_dim), amp, dtype)
@@ -217,6 +220,22 @@ def sink_ragged(seed: int = 13, dtype: str = "bf16", n_heads: int = 2, head_dim:
                          bases=bases, sink_lens=sink_lens, seed=seed, amp=amp, spare_pages=3)
 
 
+def gap_ragged(seed: int = 17, dtype: str = "bf16", n_heads: int = 2, head_dim: int = 128,
+               page_size: int = 128, amp: float = 0.5) -> Workload:
+    """Bounded "sink + local" caches whose out-of-window tokens were dropped (gap_slots, include/slack.h): a hole that
+    ends mid-tile, a hole of less than a tile with sink and window in the same 128-position tile, a hole in a one-page
+    sink, a window that still covers everything held, plus a stream without sink in the same batch."""
+    q_lens = [300, 129, 72, 257, 64]
+    cache_lens = [900, 700, 500, 1300, 300]          # held tokens (sink included)
+    windows = [700, 0, 400, 1557, 0]
+    sink_lens = [72, 200, 1, 300, 0]
+    gaps = [312, 17, 127, 84, 0]
+    bases = [0, 5, 77 % page_size, 1, 3]
+    return make_workload(f"gap_ragged_{dtype}", dtype=dtype, n_heads=n_heads, head_dim=head_dim,
+                         page_size=page_size, q_lens=q_lens, cache_lens=cache_lens, windows=windows,
+                         bases=bases, sink_lens=sink_lens, gap_slots=gaps, seed=seed, amp=amp, spare_pages=3)
+
+
 # ----------------------------------------------------------------------------------------------
 # block-sparse masks (SURVEY 8(f) NEXT-2; P:88 knob (2), rho in {0,.6,.7,.8,.9} P:568)
 # ----------------------------------------------------------------------------------------------
@@ -226,17 +245,20 @@ MASK_BLOCK_Q = 256
 MASK_BLOCK_K = 128
 
 
-def visible_key_blocks(s: StreamSpec, block_k: int = MASK_BLOCK_K) -> np.ndarray:
-    """Indices of the key blocks that hold at least one visible position of the stream (sink range, then window range)."""
+def visible_positions(s) -> np.ndarray:
+    """Positions (page-table space, include/slack.h) of the keys a stream's chunk may use: bookkeeping for placing mask
+    bits and counting flops only; the attention itself is defined in oracle/ and csrc/ separately."""
     n = s.cache_len + s.q_len
     lo = max(0, n - s.window) if s.window > 0 else 0
     sink = min(s.sink_len, n)
     lo = max(lo, sink)
-    blocks = set()
-    for a, b in ((0, sink), (lo, n)):
-        if b > a:
-            blocks.update(range((s.base + a) // block_k, (s.base + b - 1) // block_k + 1))
-    return np.array(sorted(blocks), dtype=np.int64)
+    gap = getattr(s, "gap_slots", 0)
+    return np.concatenate([s.base + np.arange(0, sink, dtype=np.int64), s.base + gap + np.arange(lo, n, dtype=np.int64)])
+
+
+def visible_key_blocks(s: StreamSpec, block_k: int = MASK_BLOCK_K) -> np.ndarray:
+    """Indices of the key blocks that hold at least one visible position of the stream (sink range, then window range)."""
+    return np.unique(visible_positions(s) // block_k)
 
 
 def random_block_masks(w: Workload, sparsity: float, seed: int = 0, block_q: int = MASK_BLOCK_Q,
@@ -252,7 +274,7 @@ def random_block_masks(w: Workload, sparsity: float, seed: int = 0, block_q: int
             masks.append(None)
             continue
         n_qb = -(-s.q_len // block_q)
-        n_kb = -(-(s.base + s.cache_len + s.q_len) // block_k)
+        n_kb = -(-(s.base + getattr(s, "gap_slots", 0) + s.cache_len + s.q_len) // block_k)
         vis = visible_key_blocks(s, block_k)
         m = np.zeros((w.n_heads, n_qb, n_kb), dtype=bool)
         n_drop = int(round(sparsity * vis.size))
@@ -272,7 +294,7 @@ def pack_block_masks(w: Workload, masks: Sequence[Optional[np.ndarray]], block_q
                      block_k: int = MASK_BLOCK_K) -> np.ndarray:
     """The mask in the layout include/slack.h asks for: uint32 [sum_s ceil(Lq_s/block_q)][H][words], bit (kb % 32) of
     word kb // 32 = key block kb; rows of a stream follow each other in stream order; a None mask packs as all ones."""
-    n_kb_max = max([-(-(s.base + s.cache_len + s.q_len) // block_k) for s in w.streams] + [1])
+    n_kb_max = max([-(-(s.base + getattr(s, "gap_slots", 0) + s.cache_len + s.q_len) // block_k) for s in w.streams] + [1])
     words = -(-n_kb_max // 32)
     rows = []
     for s, m in zip(w.streams, masks):

@@ -10,7 +10,7 @@ import torch
 
 import oracle
 from paper_2606_15319_b200 import binding
-from helpers import oracle_pools, prior_streams
+from helpers import oracle_pools, prior_batches
 
 SENTINEL_BF16 = 0x7FC1   # a NaN bit pattern: any leak of an unowned / masked slot into the output shows up as NaN
 SENTINEL_F32 = np.float32(np.nan)
@@ -35,10 +35,8 @@ def host_fill(w, sentinel=True):
 
 def gpu_append_all(ctx, w, pool, device="cuda:0", planned_plan=None):
     """Appends the prior chunks, then the new chunk, through slack_kv_append (or the planned variant for the new chunk)."""
-    if any(s.cache_len for s in w.streams):
-        kp = binding.to_torch(np.concatenate(w.k_prior), w.dtype, device)
-        vp = binding.to_torch(np.concatenate(w.v_prior), w.dtype, device)
-        ctx.slack_kv_append(pool, prior_streams(w.streams), kp, vp)
+    for descs, kk, vv in prior_batches(w):
+        ctx.slack_kv_append(pool, descs, binding.to_torch(kk, w.dtype, device), binding.to_torch(vv, w.dtype, device))
     kn = binding.to_torch(w.k_new, w.dtype, device)
     vn = binding.to_torch(w.v_new, w.dtype, device)
     if planned_plan is not None:

@@ -22,8 +22,8 @@ def hctx():
     c.close()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "slack.h")).read()
+def declared_symbols(header="slack.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(slack_[a-z_0-9]+)\s*\(", text)))
 
@@ -38,12 +38,20 @@ def test_every_declared_symbol_is_exported_and_bound():
         assert n in exported, f"{n} declared in slack.h but not exported"
         assert n in binding.SYMBOLS, f"{n} has no ctypes signature in the binding"
     lib = binding.load()
-    assert lib.slack_abi_version() == 1
+    assert lib.slack_abi_version() == 2
+    # include/slack_diag.h is exported by -DSLACK_DIAGNOSTICS builds only; the default library carries none of it
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["slack.h", "slack_diag.h"]
+    diag = declared_symbols("slack_diag.h")
+    assert diag == ["slack_debug_set"] and set(diag) == set(binding.DIAG_SYMBOLS)
+    if os.environ.get("SLACK_DIAGNOSTICS", "0") in ("", "0"):
+        assert not (set(diag) & exported), "the default build must not export the diagnostics calls"
+        ksyms = subprocess.check_output(["nm", "-C", "--defined-only", binding.LIB_PATH], text=True)
+        assert "attn_tc_kernel<true" not in ksyms, "the traced kernel instantiation must not be in the default build"
 
 
 def test_struct_sizes_match_header():
     import ctypes as C
-    assert C.sizeof(binding.CPool) == 40 and C.sizeof(binding.CStream) == 32
+    assert C.sizeof(binding.CPool) == 40 and C.sizeof(binding.CStream) == 40
     assert C.sizeof(binding.CPlanOpts) == 16 and C.sizeof(binding.CWorkItem) == 48
 
 
@@ -87,9 +95,11 @@ def check_cover(w, plan, n_cta):
         n = s.cache_len + s.q_len
         lo = max(0, n - s.window) if s.window > 0 else 0
         sink = min(getattr(s, "sink_len", 0), n)
-        if lo <= sink:                      # the window still touches the sink: one visible range
+        gap = getattr(s, "gap_slots", 0)
+        if lo <= sink and gap == 0:         # the window still touches the sink and no slot is skipped: one visible range
             lo, sink = 0, 0
-        pos_lo, pos_hi = s.base + lo, s.base + n
+        lo = max(lo, sink)
+        pos_lo, pos_hi = s.base + (gap if sink else 0) + lo, s.base + gap + n
         t0, t1 = pos_lo // 128, -(-pos_hi // 128)
         want_sink_tiles = (-(-(s.base + sink) // 128) - s.base // 128) if sink > 0 else 0
         for h in range(w.n_heads):
@@ -114,7 +124,7 @@ def check_cover(w, plan, n_cta):
 
 @pytest.mark.parametrize("splits", [0, 1, 2, 5])
 @pytest.mark.parametrize("n_cta", [1, 7, 148])
-@pytest.mark.parametrize("make", [W.small_ragged, W.sink_ragged])
+@pytest.mark.parametrize("make", [W.small_ragged, W.sink_ragged, W.gap_ragged])
 def test_plan_cover_small(hctx, splits, n_cta, make):
     w = make()
     plan = hctx.slack_plan(_pool(w), w.streams, sm_count=n_cta, force_splits=splits)
@@ -162,7 +172,7 @@ def test_kernel_kind_selection(hctx):
 
 # ------------------------------------------------------------------------------------------------ error behaviour
 def _expect(hctx, status, w, pool=None, mutate=None, **opts):
-    streams = [W.StreamSpec(s.q_len, s.cache_len, s.base, s.window, s.sink_len, s.page_table.copy()) for s in w.streams]
+    streams = [W.StreamSpec(s.q_len, s.cache_len, s.base, s.window, s.sink_len, s.page_table.copy(), s.gap_slots) for s in w.streams]
     if mutate:
         mutate(streams)
     with pytest.raises(binding.SlackError) as e:
@@ -180,6 +190,11 @@ def test_plan_rejects_malformed_descriptors(hctx):
     _expect(hctx, E, w, mutate=lambda s: s[0].page_table.__setitem__(0, -1))
     _expect(hctx, E, w, mutate=lambda s: s[1].page_table.__setitem__(0, int(s[0].page_table[0])))   # page owned twice
     _expect(hctx, E, w, mutate=lambda s: setattr(s[0], "sink_len", -4))
+    _expect(hctx, E, w, mutate=lambda s: setattr(s[0], "gap_slots", -1))
+    _expect(hctx, E, w, mutate=lambda s: setattr(s[0], "gap_slots", 5))                      # a hole needs a sink in front of it
+    def young(s):
+        s[0].sink_len, s[0].gap_slots = s[0].cache_len + 1, 5                                # ... and a filled sink
+    _expect(hctx, E, w, mutate=young)
     _expect(hctx, U, w, pool=_pool(w, head_dim=96))
     _expect(hctx, U, w, pool=_pool(w, page_size=48))
     _expect(hctx, U, w, pool=_pool(w, page_size=8))
@@ -203,7 +218,7 @@ def test_sparse_plan_geometry(hctx):
     pool = binding.Pool(None, None, w.n_pages, w.n_heads, w.head_dim, w.page_size, w.dtype)
     plan = hctx.slack_plan(pool, w.streams, force_splits=2)
     assert plan.mask_rows == sum(-(-s.q_len // 256) for s in w.streams)
-    assert plan.mask_min_words == -(-max(-(-(s.base + s.n) // 128) for s in w.streams) // 32)
+    assert plan.mask_min_words == -(-max(-(-(s.base + s.gap_slots + s.n) // 128) for s in w.streams) // 32)
     items = plan.items()
     steps = sum(it["sink_tiles"] + it["kv_tile_end"] - it["kv_tile_begin"] for it in items)
     assert plan.sparse_workspace_bytes >= plan.workspace_bytes + 2 * steps + 4 * len(items)

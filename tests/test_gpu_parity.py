@@ -91,6 +91,26 @@ def test_sink_plus_local_window_tensor_core(ctx, page_size, splits):
     assert res["kind"] == 0
 
 
+@pytest.mark.parametrize("page_size", [128, 256])
+@pytest.mark.parametrize("splits", [0, 1, 3])
+def test_bounded_sink_cache_with_hole(ctx, page_size, splits):
+    """gap_slots (include/slack.h): a "sink + local" cache whose out-of-window tokens were dropped; append lands behind the
+    hole bit-exactly and attention visits the sink tiles, skips the hole and visits the window tiles."""
+    w = W.gap_ragged(page_size=page_size)
+    pool = G.make_pool(w)
+    G.gpu_append_all(ctx, w, pool)
+    assert G.pools_equal_oracle(w, pool)
+    res, *_ = run_case(ctx, w, force_splits=splits)
+    assert res["kind"] == 0
+
+
+def test_bounded_sink_cache_with_hole_simt(ctx):
+    res, *_ = run_case(ctx, W.gap_ragged(dtype="f32", head_dim=64, page_size=16), tol=(1e-5, 1e-5))
+    assert res["kind"] == 1
+    res, *_ = run_case(ctx, W.gap_ragged(), force_simt=1)
+    assert res["kind"] == 1
+
+
 def test_sink_plus_local_window_simt(ctx):
     res, *_ = run_case(ctx, W.sink_ragged(dtype="f32", head_dim=64, page_size=16), tol=(1e-5, 1e-5))
     assert res["kind"] == 1
@@ -218,3 +238,46 @@ def test_unusual_shapes_sampled_rows(ctx, n_heads, page_size, lq, lc, window, ba
     for splits in (0, 1):
         res, out, *_ = run_case(ctx, w, rows=rows, force_splits=splits)
         assert res["kind"] == 0
+
+
+# ------------------------------------------------------------------------------------------------ plan / staging lifetime
+def test_plans_created_and_destroyed_while_kernels_are_in_flight(ctx):
+    """slack_plan takes its tables from the ctx arena and slack_plan_destroy hands them back through events: hundreds of
+    plans are made, used once on one of two streams and destroyed at once (no synchronisation in between); every output
+    must equal the one computed with a long-lived plan, bit for bit."""
+    w = W.small_ragged(page_size=256)
+    pool = G.make_pool(w)
+    G.gpu_append_all(ctx, w, pool)
+    ref, _, plan0, _ = G.gpu_attention(ctx, w, pool, force_splits=2)
+    q = binding.to_torch(w.q, w.dtype, "cuda:0")
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [torch.full_like(q, float("nan")) for _ in range(2)]
+    wss = [torch.empty(max(plan0.workspace_bytes, 16), dtype=torch.uint8, device="cuda:0") for _ in range(2)]
+    torch.cuda.synchronize()
+    for it in range(300):
+        st = streams[it & 1]
+        plan = ctx.slack_plan(pool, w.streams, force_splits=2)
+        ctx.slack_chunk_attention(plan, pool, q, outs[it & 1], w.scale, workspace=wss[it & 1], stream=st)
+        plan.close()
+    torch.cuda.synchronize()
+    for o in outs:
+        assert np.array_equal(o.float().cpu().numpy().astype(np.float64), ref)
+
+
+def test_unplanned_appends_on_two_streams_do_not_share_staging(ctx):
+    """two slack_kv_append calls back to back on different streams used to share one staging table."""
+    wa, wb = W.small_ragged(seed=41, page_size=256), W.small_ragged(seed=42, page_size=256)
+    pa, pb = G.make_pool(wa), G.make_pool(wb)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    ka, va = binding.to_torch(wa.k_new, wa.dtype, "cuda:0"), binding.to_torch(wa.v_new, wa.dtype, "cuda:0")
+    kb, vb = binding.to_torch(wb.k_new, wb.dtype, "cuda:0"), binding.to_torch(wb.v_new, wb.dtype, "cuda:0")
+    torch.cuda.synchronize()
+    for _ in range(20):
+        ctx.slack_kv_append(pa, wa.streams, ka, va, stream=sa)
+        ctx.slack_kv_append(pb, wb.streams, kb, vb, stream=sb)
+    torch.cuda.synchronize()
+    import helpers
+    for w, pool in ((wa, pa), (wb, pb)):
+        ko, vo = helpers.empty_pools(w, G.host_fill(w))
+        oracle.kv_append(ko, vo, w.streams, w.k_new, w.v_new)
+        assert np.array_equal(binding.to_numpy(pool.k_pool, w.dtype), ko) and np.array_equal(binding.to_numpy(pool.v_pool, w.dtype), vo)

@@ -149,3 +149,38 @@ def test_transfer_argument_errors(ctx):
         ctx.slack_kv_transfer([src], [dst], ids, ids, 1, 1)                                                # empty head range
     ctx.slack_kv_transfer([src], [dst], ids[:0], ids[:0], 0, w.n_heads)                                     # empty list: no-op
     assert ctx.last_launch_count == 0
+
+
+def test_back_to_back_transfers_on_two_streams(ctx):
+    """the page-id lists of a transfer are staged per call and released behind its last kernel, so two
+    transfers queued back to back on different streams cannot overwrite each other's lists."""
+    w = W.small_ragged(page_size=256)
+    src = G.make_pool(w)
+    G.gpu_append_all(ctx, w, src)
+    ko, vo = oracle_pools(w, fill=G.host_fill(w))
+    s0, s1 = w.streams[0], w.streams[3]
+    sp0, sp1 = np.asarray(s0.page_table, np.int32), np.asarray(s1.page_table, np.int32)
+    n_dst = int(sp0.size + sp1.size + 3)
+    dst, dk, dv = sentinel_pool(w, n_dst)
+    perm = np.random.default_rng(9).permutation(n_dst).astype(np.int32)
+    dp0, dp1 = perm[:sp0.size], perm[sp0.size:sp0.size + sp1.size]
+    a, b = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(10):
+        ctx.slack_kv_transfer([src] * 4, [dst] * 4, sp0, dp0, 0, w.n_heads, stream=a)
+        ctx.slack_kv_transfer([src] * 4, [dst] * 4, sp1, dp1, 0, w.n_heads, stream=b)
+    torch.cuda.synchronize()
+    oracle.kv_transfer(ko, vo, dk, dv, sp0, dp0, 0, w.n_heads)
+    oracle.kv_transfer(ko, vo, dk, dv, sp1, dp1, 0, w.n_heads)
+    assert np.array_equal(bits(binding.to_numpy(dst.k_pool, w.dtype)), bits(dk))
+    assert np.array_equal(bits(binding.to_numpy(dst.v_pool, w.dtype)), bits(dv))
+
+
+def test_transfer_inside_one_pool_rejects_read_write_overlap(ctx):
+    w = W.small_ragged(page_size=256)
+    pool = G.make_pool(w)
+    ids = np.asarray(w.streams[0].page_table, np.int32)
+    assert ids.size >= 2
+    with pytest.raises(binding.SlackError) as e:
+        ctx.slack_kv_transfer([pool], [pool], ids[:2], ids[1:3] if ids.size >= 3 else ids[::-1][:2], 0, w.n_heads)
+    assert e.value.status == binding.SLACK_EINVAL

@@ -43,6 +43,8 @@ def brute_force(w, k_pool, v_pool):
                 vals = []
                 for t in keys:
                     pos = s.base + t
+                    if t >= s.sink_len:
+                        pos += s.gap_slots               # hole behind the sink left by dropped tokens (slack.h)
                     page = int(s.page_table[pos // P])
                     slot = pos % P
                     kv = [dec(k_pool[page, h, slot, d]) for d in range(D)]
