@@ -36,11 +36,8 @@ def _rank_main(rank, world, port, out_q):
     flops = metrics.attention_flops(w.streams, w.n_heads, w.head_dim)
     fake_ms = 10.0 + 5.0 * rank                                   # stands in for the rank's CUDA-event time
     dist.barrier()
-    t = torch.tensor([fake_ms], dtype=torch.float64)
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    f = torch.tensor([flops], dtype=torch.float64)
-    dist.all_reduce(f, op=dist.ReduceOp.SUM)
-    out_q.put((rank, plan.num_items, [s.cache_len for s in w.streams], flops, float(t.item()), float(f.item())))
+    t, f = bench.reduce_job(dist, fake_ms, flops)               # the very reduction bench.py's `value` is built from
+    out_q.put((rank, plan.num_items, [s.cache_len for s in w.streams], flops, t, f))
     dist.barrier()
     dist.destroy_process_group()
 
