@@ -56,6 +56,8 @@ def parse_args():
     ap.add_argument("--kv-chunks", type=int, default=7, help="cfg5: visible chunks (1..7)")
     ap.add_argument("--layers", type=int, default=30)
     ap.add_argument("--force-splits", type=int, default=0)
+    ap.add_argument("--cta-pairs", type=int, default=0, choices=[0, 1, 2],
+                    help="slack_plan_opts.cta_pairs: 0 = automatic, 1 = one CTA per item, 2 = CTA pairs (cta_group::2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -297,7 +299,7 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
         qs.append(rnd(tq, H, D)); kns.append(rnd(tq, H, D)); vns.append(rnd(tq, H, D))
         outs.append(torch.empty(tq, H, D, device=dev, dtype=torch.bfloat16))
     main = torch.cuda.current_stream()
-    plan0 = ctx.slack_plan(pools[0], w.streams, force_splits=args.force_splits)
+    plan0 = ctx.slack_plan(pools[0], w.streams, force_splits=args.force_splits, cta_pairs=args.cta_pairs)
     ws = torch.empty(max(plan0.workspace_bytes, plan0.sparse_workspace_bytes if sparsity > 0 else 0, 256),
                      dtype=torch.uint8, device=dev)
     # block-sparse variant: a seeded mask per layer (the selection rule, Light Forcing's [39] P:319, is outside the path)
@@ -313,7 +315,7 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
     def step(q_of=lambda l: qs[l], kn_of=lambda l: kns[l], vn_of=lambda l: vns[l], out_of=lambda l: outs[l],
              pre=lambda l: None, post=lambda l: None):
         t0 = time.perf_counter()
-        plan = ctx.slack_plan(pools[0], w.streams, force_splits=args.force_splits)      # A0 + A2 (host), once per step
+        plan = ctx.slack_plan(pools[0], w.streams, force_splits=args.force_splits, cta_pairs=args.cta_pairs)      # A0 + A2 (host), once per step
         state["plan_s"] += time.perf_counter() - t0
         for l in range(L):
             pre(l)

@@ -102,7 +102,9 @@ typedef struct {
                            exactly min(k, #kv tiles) parts (1 = never split)                                     */
   int32_t force_simt;   /* 1 = plan for the fp32-accumulating SIMT validation kernel even where the tensor-core path
                            applies (debug / cross-check); f32 pools always use it                                */
-  int32_t reserved;
+  int32_t cta_pairs;    /* tensor-core path: 0 = automatic, 1 = one CTA per work item, 2 = CTA pairs (two SMs walk a
+                           work item together, 128 query rows each, and share every K/V tile: tcgen05 cta_group::2;
+                           the plan then has sm_count / 2 queues; needs an even sm_count)                       */
 } slack_plan_opts;
 
 /* One unit of attention work as planned (inspection only; see slack_plan_get_items). Key tiles are 128 pool slots,
@@ -121,7 +123,7 @@ typedef struct {
                             first piece of a split row carries them), starting at tile base / 128                  */
   int32_t sink_pos_hi;   /* base + sink_len when the item visits sink tiles, else base                            */
   int32_t partial_slot;  /* -1: writes `out` directly; >= 0: writes workspace slot (split-KV), combined afterwards */
-  int32_t cta;           /* CTA (0..sm_count-1) whose queue holds this item                                      */
+  int32_t cta;           /* queue that holds this item: CTA 0..sm_count-1, or CTA pair 0..sm_count/2-1 (pair plans) */
 } slack_work_item;
 
 /* ---- context ------------------------------------------------------------------------------------------------ */
@@ -154,7 +156,8 @@ void slack_plan_destroy(slack_plan_t *plan);
 size_t slack_plan_workspace_bytes(const slack_plan_t *plan); /* device bytes slack_chunk_attention needs (may be 0) */
 int32_t slack_plan_num_items(const slack_plan_t *plan);
 int32_t slack_plan_num_partial_slots(const slack_plan_t *plan);
-int32_t slack_plan_kernel_kind(const slack_plan_t *plan);    /* 0 = tcgen05 tensor-core kernel, 1 = SIMT kernel */
+int32_t slack_plan_kernel_kind(const slack_plan_t *plan);    /* 0 = tcgen05 kernel, one CTA per item; 1 = SIMT kernel;
+                                                                2 = tcgen05 kernel, CTA pairs                      */
 /* Copies up to `capacity` planned items (in queue order) to `items`; returns how many were written. */
 int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, int32_t capacity);
 

@@ -39,7 +39,7 @@ class CStream(C.Structure):
 
 
 class CPlanOpts(C.Structure):
-    _fields_ = [("sm_count", C.c_int32), ("force_splits", C.c_int32), ("force_simt", C.c_int32), ("reserved", C.c_int32)]
+    _fields_ = [("sm_count", C.c_int32), ("force_splits", C.c_int32), ("force_simt", C.c_int32), ("cta_pairs", C.c_int32)]
 
 
 class CWorkItem(C.Structure):
@@ -238,9 +238,9 @@ class Context:
 
     # --- the three calls of the boundary, same names as the C ABI ---------------------------------------------------
     def slack_plan(self, pool: Pool, streams: Sequence, sm_count: int = 0, force_splits: int = 0,
-                   force_simt: int = 0) -> Plan:
+                   force_simt: int = 0, cta_pairs: int = 0) -> Plan:
         arr, keep = _stream_array(streams)
-        opts = CPlanOpts(sm_count, force_splits, force_simt, 0)
+        opts = CPlanOpts(sm_count, force_splits, force_simt, cta_pairs)
         h = _VP()
         self._check(self.lib.slack_plan(self.handle, C.byref(pool.c), len(streams), arr, C.byref(opts), C.byref(h)))
         del keep

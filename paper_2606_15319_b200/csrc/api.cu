@@ -742,12 +742,15 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   if (!ctx->encode) return set_err(ctx, SLACK_ECUDA, "cuTensorMapEncodeTiled entry point not available");
   if (!ctx->tc_configured) {
     SLACK_CUDA(ctx, attn_tc_configure());
+    SLACK_CUDA(ctx, attn_tc2_configure());
     ctx->tc_configured = true;
   }
+  // pair plans run on CTA pairs (attn_tc2.cu); the block-sparse call walks the same items one CTA at a time
+  const bool pairs = hp.kernel_kind == 2 && !block_mask;
   CUtensorMap tm_q, tm_k, tm_v;
   const uint64_t pool_rows = (uint64_t)hp.n_pages * hp.n_heads * hp.page_size;
   if ((st = make_map(ctx, &tm_q, q, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
-  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows, pairs ? 64 : 128)) != SLACK_OK) return st;
   if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
   if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
   TcParams p{};
@@ -781,7 +784,10 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   }
   cudaEvent_t ev_after;
   if ((st = prof_begin(ctx, 0, cs, &ev_after)) != SLACK_OK) return st;
-  SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_cta, cs, &ctx->last_launches));
+  if (pairs)
+    SLACK_CUDA(ctx, launch_attn_tc2(p, tm_q, tm_k, tm_v, 2 * hp.n_queues, cs, &ctx->last_launches));
+  else
+    SLACK_CUDA(ctx, launch_attn_tc(p, tm_q, tm_k, tm_v, hp.n_queues, cs, &ctx->last_launches));
   if ((st = prof_end(ctx, 0, cs, ev_after)) != SLACK_OK) return st;
   if (!hp.combines.empty()) {
     if ((st = prof_begin(ctx, 2, cs, &ev_after)) != SLACK_OK) return st;

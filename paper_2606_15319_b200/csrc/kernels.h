@@ -70,6 +70,12 @@ cudaError_t attn_tc_configure(); // cudaFuncSetAttribute(max dynamic smem); once
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched);
 
+// A3 on CTA pairs (attn_tc2.cu, tcgen05 cta_group::2): needs a pair plan (HostPlan::kernel_kind 2, even n_cta) and a K
+// tensor map with 64-row boxes (each CTA loads half of a key tile's keys).
+cudaError_t attn_tc2_configure();
+cudaError_t launch_attn_tc2(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
+                            int n_cta, cudaStream_t st, int *n_launched);
+
 // Block-sparse A3: per item, the selected key-tile steps under a device block mask (see sparse_steps.cu).
 cudaError_t launch_sparse_steps(const DevItem *d_items, int n_items, const uint32_t *mask, int n_heads, int mask_words,
                                 uint16_t *steps, int32_t *count, cudaStream_t st, int *n_launched);

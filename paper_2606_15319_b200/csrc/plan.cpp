@@ -122,6 +122,7 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
 // tail rows produce split-KV partials.  (Cutting every queue's share out of one line - plain stream-K - balances as
 // well but de-synchronises the sweeps: measured 17 % slower on BASELINE config 5, its K/V working set leaving L2.)
 constexpr int32_t kMinPiece = 4;
+constexpr bool kAutoPairs = false; // automatic plans use CTA pairs where they pay (see build_plan)
 constexpr double kTileCost1 = 1.55; // one 128-key tile against a single query tile: measured 2620 vs 3400 cycles (the chain bounds it)
 
 struct Row {
@@ -130,7 +131,7 @@ struct Row {
 };
 
 void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevStream> &ds, int32_t n_heads, int32_t n_cta,
-                   double target_scale, Candidate &c) {
+                   bool pairs, double target_scale, Candidate &c) {
   c = Candidate();
   std::vector<Row> rows;
   double total = 0;
@@ -147,7 +148,7 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
         r.tile0 = g.tile0;
         r.tiles = g.tiles;
         r.sink_tiles = g.sink_tiles;
-        r.tc = r.q_rows > kTileM ? kTileCost : kTileCost1;
+        r.tc = (pairs || r.q_rows > kTileM) ? kTileCost : kTileCost1; // a CTA pair moves at one pace whatever the odd CTA holds
         total += r.tc * (r.tiles + r.sink_tiles) + kItemOverhead;
         rows.push_back(r);
       }
@@ -274,6 +275,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   out.n_streams = n_streams;
   out.n_cta = opts.sm_count > 0 ? opts.sm_count : default_sm_count;
   const bool tc_ok = shape.dtype == SLACK_BF16 && shape.head_dim == 128 && shape.page_size >= kTileN;
+  if (opts.cta_pairs < 0 || opts.cta_pairs > 2) return fail(SLACK_EINVAL, "plan opts: cta_pairs must be 0, 1 or 2");
   out.kernel_kind = (tc_ok && !opts.force_simt) ? 0 : 1;
 
   // ---- validate streams, build device stream records and the concatenated page table ------------------------
@@ -351,6 +353,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   out.total_q = (int32_t)row;
   if (out.page_tables.empty()) out.page_tables.push_back(0); // keep device arrays non-empty
 
+  out.n_queues = out.n_cta;
   out.cta_begin.assign((size_t)out.n_cta + 1, 0);
   if (out.kernel_kind == 1) return SLACK_OK; // the SIMT kernel walks DevStream records directly: no items
 
@@ -372,6 +375,26 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
                    [](const StreamGeom &a, const StreamGeom &b) { return a.tiles + a.sink_tiles > b.tiles + b.sink_tiles; });
   if (order.empty()) return SLACK_OK;
 
+  // CTA pairs (attn_tc2.cu, tcgen05 cta_group::2): two SMs walk ONE queue together, each item's first 128 query rows on
+  // the even CTA and the rest on the odd one, and share every K/V tile.  The plan is then made for n_cta / 2 queues.
+  // Pays when most items have more than 128 rows; short chunks (decode-like) keep one CTA per item.
+  // cta_pairs: 0 = automatic, 1 = never, 2 = always (needs an even CTA count).
+  if (out.n_cta >= 2 && out.n_cta % 2 == 0) {
+    bool pairs = opts.cta_pairs == 2;
+    if (opts.cta_pairs == 0 && kAutoPairs) {
+      int64_t rows = 0, padded = 0;
+      for (const StreamGeom &g : order) {
+        rows += out.streams[g.idx].q_len;
+        padded += (int64_t)g.q_blocks * kItemRows;
+      }
+      pairs = rows * 100 >= padded * 85; // at least 85 % of the items' 256 query slots are real queries
+    }
+    if (pairs) out.kernel_kind = 2;
+  }
+  const int32_t n_queues = out.kernel_kind == 2 ? out.n_cta / 2 : out.n_cta;
+  out.n_queues = n_queues;
+  out.cta_begin.assign((size_t)n_queues + 1, 0);
+
   const int32_t t_max = order.front().tiles;
   Candidate best;
   bool have = false;
@@ -386,7 +409,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
       }
     }
     Candidate c;
-    make_candidate(order, parts, out.streams, shape.n_heads, out.n_cta, c);
+    make_candidate(order, parts, out.streams, shape.n_heads, n_queues, c);
     if (!have || c.objective < best.objective - 1e-9) {
       best = std::move(c);
       have = true;
@@ -400,16 +423,16 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     const double scales[] = {1.0, 0.99, 1.01, 0.98, 1.02, 0.97, 1.03, 1.045, 1.06};
     for (double sc : scales) {
       Candidate c;
-      make_balanced(order, out.streams, shape.n_heads, out.n_cta, sc, c);
+      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, sc, c);
       if (c.objective < best.objective - 1e-9) best = std::move(c);
     }
   }
 
   // ---- emit per-CTA queues (stable: queue order = item order) ------------------------------------------------
   const size_t n_items = best.items.size();
-  std::vector<int32_t> count((size_t)out.n_cta, 0);
+  std::vector<int32_t> count((size_t)n_queues, 0);
   for (size_t i = 0; i < n_items; ++i) count[best.item_cta[i]]++;
-  for (int32_t c = 0; c < out.n_cta; ++c) out.cta_begin[c + 1] = out.cta_begin[c] + count[c];
+  for (int32_t c = 0; c < n_queues; ++c) out.cta_begin[c + 1] = out.cta_begin[c] + count[c];
   std::vector<int32_t> cursor(out.cta_begin.begin(), out.cta_begin.end() - 1);
   out.items.resize(n_items);
   out.item_cta.resize(n_items);

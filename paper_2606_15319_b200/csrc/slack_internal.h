@@ -80,11 +80,12 @@ struct HostPlan {
   int32_t n_pages = 0, n_heads = 0, head_dim = 0, page_size = 0, dtype = 0;
   int32_t n_streams = 0, total_q = 0;
   int32_t n_cta = 0;
-  int32_t kernel_kind = 0; // 0 tensor-core, 1 SIMT
+  int32_t n_queues = 0;    // item queues: n_cta, or n_cta / 2 for pair plans
+  int32_t kernel_kind = 0; // 0 tensor-core (one CTA per queue), 1 SIMT, 2 tensor-core CTA pairs (n_cta / 2 queues, cta_group::2)
   std::vector<DevStream> streams;
   std::vector<int32_t> page_tables;  // concatenated
   std::vector<DevItem> items;        // in queue order: CTA c owns items [cta_begin[c], cta_begin[c+1])
-  std::vector<int32_t> cta_begin;    // n_cta + 1
+  std::vector<int32_t> cta_begin;    // queues + 1 (queues = n_cta, or n_cta / 2 for pair plans)
   std::vector<int32_t> item_cta;     // per item
   std::vector<DevCombine> combines;
   int32_t n_partial_slots = 0;

@@ -5,6 +5,8 @@ from the same seeded Workload arrays (paper_2606_15319_b200.workloads).
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import torch
 
@@ -52,6 +54,8 @@ def make_pool(w, device="cuda:0", sentinel=True):
 
 
 def gpu_attention(ctx, w, pool, device="cuda:0", want_lse=True, **plan_opts):
+    # SLACK_TEST_CTA_PAIRS=1|2 reruns every case that does not choose itself on one CTA per item / on CTA pairs
+    plan_opts.setdefault("cta_pairs", int(os.environ.get("SLACK_TEST_CTA_PAIRS", "0")))
     plan = ctx.slack_plan(pool, w.streams, **plan_opts)
     q = binding.to_torch(w.q, w.dtype, device)
     out = torch.full_like(q, float("nan"))

@@ -122,14 +122,17 @@ def check_cover(w, plan, n_cta):
     return items
 
 
+@pytest.mark.parametrize("pairs", [1, 2])
 @pytest.mark.parametrize("splits", [0, 1, 2, 5])
-@pytest.mark.parametrize("n_cta", [1, 7, 148])
+@pytest.mark.parametrize("n_cta", [1, 7, 8, 148])
 @pytest.mark.parametrize("make", [W.small_ragged, W.sink_ragged, W.gap_ragged])
-def test_plan_cover_small(hctx, splits, n_cta, make):
+def test_plan_cover_small(hctx, splits, n_cta, make, pairs):
+    """cta_pairs = 2 (include/slack.h): the same items, dealt to sm_count / 2 queues, one per CTA pair."""
     w = make()
-    plan = hctx.slack_plan(_pool(w), w.streams, sm_count=n_cta, force_splits=splits)
-    assert plan.kernel_kind == 0
-    check_cover(w, plan, n_cta)
+    plan = hctx.slack_plan(_pool(w), w.streams, sm_count=n_cta, force_splits=splits, cta_pairs=pairs)
+    paired = pairs == 2 and n_cta % 2 == 0                      # an odd CTA count cannot pair up
+    assert plan.kernel_kind == (2 if paired else 0)
+    check_cover(w, plan, n_cta // 2 if paired else n_cta)
     if splits == 1:
         assert plan.num_partial_slots == 0 and plan.workspace_bytes == 0
     else:
@@ -143,14 +146,16 @@ def _descr_only(maker):
         return maker()
 
 
+@pytest.mark.parametrize("pairs", [1, 2])
 @pytest.mark.parametrize("maker", [W.config2, W.config3, W.config4, lambda: W.config5(7), lambda: W.config5(1), W.config5b])
-def test_plan_cover_and_balance_full_configs(hctx, maker):
+def test_plan_cover_and_balance_full_configs(hctx, maker, pairs):
     w = _descr_only(maker)
-    plan = hctx.slack_plan(_pool(w), w.streams, sm_count=148)
-    items = check_cover(w, plan, 148)
-    load = np.zeros(148)
+    plan = hctx.slack_plan(_pool(w), w.streams, sm_count=148, cta_pairs=pairs)
+    nq = 148 // pairs
+    items = check_cover(w, plan, nq)
+    load = np.zeros(nq)
     for it in items:
-        load[it["cta"]] += (2.0 if it["q_rows"] > 128 else 1.55) * (it["kv_tile_end"] - it["kv_tile_begin"]) + 9.0
+        load[it["cta"]] += (2.0 if (pairs == 2 or it["q_rows"] > 128) else 1.55) * (it["kv_tile_end"] - it["kv_tile_begin"]) + 9.0
     assert load.max() <= 1.25 * load.mean() + 40, f"{w.name}: makespan {load.max():.0f} vs ideal {load.mean():.0f}"
 
 
