@@ -73,6 +73,9 @@ def to_f64(x: np.ndarray, dtype: str) -> np.ndarray:
     if dtype == "f32":
         assert x.dtype == np.float32
         return x.astype(np.float64)
+    if dtype == "f64":          # already-widened operands (oracle/fp8_attention.py hands dequantised values in)
+        assert x.dtype == np.float64
+        return x
     raise ValueError(dtype)
 
 

@@ -68,3 +68,20 @@ def stream_rows(w):
         out.append((r, r + s.q_len))
         r += s.q_len
     return out
+
+
+def oracle_pools_fp8(w, code_fill=0x7F, scale_fill=np.nan, with_new=True):
+    """FP8 pool image (codes uint8 [n_pages, H, P, D] + fp32 scales [n_pages, H, P // 128], K and V) after the oracle's
+    quantising append of the prior chunks (and, if with_new, the new chunk).  Unwritten slots keep `code_fill` (0x7f =
+    NaN) and untouched scales `scale_fill`."""
+    F = oracle.fp8_attention
+    shape = (w.n_pages, w.n_heads, w.page_size, w.head_dim)
+    kc = np.full(shape, code_fill, dtype=np.uint8)
+    vc = kc.copy()
+    ks = np.full((w.n_pages, w.n_heads, w.page_size // F.KEY_BLOCK), scale_fill, dtype=np.float32)
+    vs = ks.copy()
+    for descs, kk, vv in prior_batches(w):
+        F.kv_append_fp8(kc, vc, ks, vs, descs, kk, vv, w.dtype)
+    if with_new:
+        F.kv_append_fp8(kc, vc, ks, vs, w.streams, w.k_new, w.v_new, w.dtype)
+    return kc, vc, ks, vs
