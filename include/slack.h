@@ -47,19 +47,29 @@
 extern "C" {
 #endif
 
-#define SLACK_ABI_VERSION 2
+#define SLACK_ABI_VERSION 3
 
 typedef enum {
   SLACK_OK = 0,
   SLACK_EINVAL = 1,       /* malformed descriptors: negative lengths, base >= page_size, short page table, page id out of
                              range, a physical page owned twice in the batch, misaligned (<16 B) pointer, NULL argument */
-  SLACK_EUNSUPPORTED = 2, /* valid but not built: head_dim not in {64,128}, page_size not a power of two >= 16 */
+  SLACK_EUNSUPPORTED = 2, /* valid but not built: head_dim not in {64,128}, page_size not a power of two >= 16; FP8 pools
+                             with head_dim != 128, page_size < 128, force_simt, the block-sparse call or slack_kv_transfer */
   SLACK_ENOMEM = 3,       /* host or device allocation failed, or workspace_bytes too small */
   SLACK_ECUDA = 4,        /* a CUDA runtime/driver call failed, or the context has no device */
   SLACK_ESTALE_PLAN = 5   /* plan does not match the pool shape / dtype passed with it */
 } slack_status;
 
-typedef enum { SLACK_BF16 = 0, SLACK_F32 = 1 } slack_dtype;
+/* SLACK_FP8_E4M3 is a POOL dtype only (PAPER.md P:88 knob (4) "quantization mode Q", Q in {FP16, FP8}
+ * P:568; "online FP8 attention quantization ... without quantizing model weights").  Such a pool holds OCP e4m3 codes
+ * (1 byte per element, same [n_pages][n_heads][page_size][head_dim] layout) plus one fp32 scale per (page, head, 128-slot
+ * key block) for K and for V; q, k_new, v_new and out stay bf16.  Quantisation rule (reading A19; the oracle
+ * states it in full): code = e4m3(x / scale), round to nearest even, saturating at +-448, both divisions in IEEE fp32;
+ * scale = amax / 448 over the tokens the append writes into the block (all of head_dim; amax = 0 -> 1); an append SETS
+ * a block's scale iff none of the stream's earlier tokens [0, cache_len) lies in that block, otherwise it keeps the
+ * stored scale.  Inside the attention call Q is quantised per (row, head) and P per element (e4m3); accumulation fp32. */
+typedef enum { SLACK_BF16 = 0, SLACK_F32 = 1, SLACK_FP8_E4M3 = 2 } slack_dtype;
+#define SLACK_SCALE_BLOCK 128 /* slots per K/V scale of an FP8 pool = the key tile of slack_work_item */
 
 typedef struct slack_ctx slack_ctx;   /* opaque */
 typedef struct slack_plan_s slack_plan_t; /* opaque */
@@ -71,7 +81,10 @@ typedef struct {
   void *k_pool;
   void *v_pool;
   int32_t n_pages, n_heads, head_dim, page_size;
-  int32_t dtype; /* slack_dtype */
+  int32_t dtype;    /* slack_dtype */
+  int32_t reserved; /* 0 */
+  float *k_scale;   /* SLACK_FP8_E4M3 pools: DEVICE fp32 [n_pages][n_heads][page_size / 128], written by slack_kv_append, */
+  float *v_scale;   /* read by slack_chunk_attention; NULL (ignored) for the other dtypes                                */
 } slack_pool;
 
 /* One stream of the batch; HOST memory. */
@@ -163,7 +176,8 @@ int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, i
 
 /* ---- A3 + A4: chunk attention and split-KV combine ------------------------------------------------------------ */
 /* Precondition: the own chunk's K/V is already appended (pool holds logical tokens [0, Lc+Lq) of every stream).
- * q, out: DEVICE [sum Lq][n_heads][head_dim] of the pool dtype (16-byte aligned; 128-byte for the bf16 path);
+ * q, out: DEVICE [sum Lq][n_heads][head_dim] of the pool dtype, bf16 for FP8 pools (16-byte aligned; 128-byte for the
+ * tensor-core paths);
  * lse: optional DEVICE fp32 [n_heads][sum Lq] (natural log), may be NULL; workspace: DEVICE, >=
  * slack_plan_workspace_bytes(plan) bytes, 16-byte aligned, may be NULL when that is 0.  Asynchronous on cuda_stream. */
 slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q,

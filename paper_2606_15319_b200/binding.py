@@ -17,8 +17,8 @@ LIB_PATH = os.path.join(_PKG_DIR, "libslack.so")
 
 SLACK_OK, SLACK_EINVAL, SLACK_EUNSUPPORTED, SLACK_ENOMEM, SLACK_ECUDA, SLACK_ESTALE_PLAN = range(6)
 STATUS_NAMES = ["SLACK_OK", "SLACK_EINVAL", "SLACK_EUNSUPPORTED", "SLACK_ENOMEM", "SLACK_ECUDA", "SLACK_ESTALE_PLAN"]
-SLACK_BF16, SLACK_F32 = 0, 1
-DTYPES = {"bf16": SLACK_BF16, "f32": SLACK_F32}
+SLACK_BF16, SLACK_F32, SLACK_FP8_E4M3 = 0, 1, 2
+DTYPES = {"bf16": SLACK_BF16, "f32": SLACK_F32, "fp8": SLACK_FP8_E4M3}
 
 
 class SlackError(RuntimeError):
@@ -29,7 +29,8 @@ class SlackError(RuntimeError):
 
 class CPool(C.Structure):
     _fields_ = [("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("n_pages", C.c_int32), ("n_heads", C.c_int32),
-                ("head_dim", C.c_int32), ("page_size", C.c_int32), ("dtype", C.c_int32)]
+                ("head_dim", C.c_int32), ("page_size", C.c_int32), ("dtype", C.c_int32), ("reserved", C.c_int32),
+                ("k_scale", C.c_void_p), ("v_scale", C.c_void_p)]
 
 
 class CStream(C.Structure):
@@ -143,11 +144,14 @@ def _cuda_stream(stream) -> Optional[int]:
 
 
 class Pool:
-    """One layer's K/V pool: torch tensors [n_pages, H, P, D] (bf16 or f32), caller-owned."""
+    """One layer's K/V pool: torch tensors [n_pages, H, P, D] (bf16 or f32), caller-owned.  dtype "fp8": uint8 tensors of
+    e4m3 codes plus k_scale / v_scale, fp32 [n_pages, H, P // 128] (include/slack.h slack_dtype)."""
 
-    def __init__(self, k_pool, v_pool, n_pages: int, n_heads: int, head_dim: int, page_size: int, dtype: str):
-        self.k_pool, self.v_pool = k_pool, v_pool
-        self.c = CPool(_ptr(k_pool), _ptr(v_pool), n_pages, n_heads, head_dim, page_size, DTYPES[dtype])
+    def __init__(self, k_pool, v_pool, n_pages: int, n_heads: int, head_dim: int, page_size: int, dtype: str,
+                 k_scale=None, v_scale=None):
+        self.k_pool, self.v_pool, self.k_scale, self.v_scale = k_pool, v_pool, k_scale, v_scale
+        self.c = CPool(_ptr(k_pool), _ptr(v_pool), n_pages, n_heads, head_dim, page_size, DTYPES[dtype], 0,
+                       _ptr(k_scale), _ptr(v_scale))
 
     @classmethod
     def shape_only(cls, n_pages, n_heads, head_dim, page_size, dtype):

@@ -17,7 +17,7 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 INCLUDE = os.path.join(os.path.dirname(PKG_DIR), "include")
 LIB_PATH = os.path.join(PKG_DIR, "libslack.so")
-SOURCES = ["api.cu", "plan.cpp", "pager.cpp", "append.cu", "attn_simt.cu", "attn_tc.cu", "attn_tc2.cu", "combine.cu", "sparse_steps.cu", "transfer.cu"]
+SOURCES = ["api.cu", "plan.cpp", "pager.cpp", "append.cu", "attn_simt.cu", "attn_tc.cu", "attn_tc2.cu", "combine.cu", "sparse_steps.cu", "transfer.cu", "quant.cu"]
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 

@@ -227,18 +227,22 @@ slack_status ensure_device(slack_ctx *ctx) {
 slack_status check_pool(slack_ctx *ctx, const slack_pool *pool, const HostPlan *hp) {
   if (!pool || !pool->k_pool || !pool->v_pool) return set_err(ctx, SLACK_EINVAL, "pool or pool pointers NULL");
   if (!aligned(pool->k_pool, 16) || !aligned(pool->v_pool, 16)) return set_err(ctx, SLACK_EINVAL, "pool pointers must be 16-byte aligned");
+  if (pool->dtype == SLACK_FP8_E4M3 && (!pool->k_scale || !pool->v_scale || !aligned(pool->k_scale, 4) || !aligned(pool->v_scale, 4)))
+    return set_err(ctx, SLACK_EINVAL, "FP8 pool: k_scale / v_scale NULL or misaligned");
   if (hp && (pool->n_pages != hp->n_pages || pool->n_heads != hp->n_heads || pool->head_dim != hp->head_dim ||
              pool->page_size != hp->page_size || pool->dtype != hp->dtype))
     return set_err(ctx, SLACK_ESTALE_PLAN, "plan was made for a different pool shape / dtype");
   return SLACK_OK;
 }
 
-slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t cols, uint64_t rows, uint32_t box_rows = 128) {
+// 2-D map over [rows][cols] elements with boxes of 128 bytes x box_rows rows (bf16: 64 elements, e4m3 codes: 128)
+slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t cols, uint64_t rows, uint32_t box_rows = 128,
+                      bool bytes = false) {
   const cuuint64_t dims[2] = {cols, rows};
-  const cuuint64_t strides[1] = {cols * 2};
-  const cuuint32_t box[2] = {64, box_rows};
+  const cuuint64_t strides[1] = {cols * (bytes ? 1 : 2)};
+  const cuuint32_t box[2] = {bytes ? 128u : 64u, box_rows};
   const cuuint32_t estr[2] = {1, 1};
-  CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+  CUresult r = ctx->encode(m, bytes ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
@@ -249,7 +253,7 @@ slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t
   return SLACK_OK;
 }
 
-int elem_bytes(int dtype) { return dtype == SLACK_BF16 ? 2 : 4; }
+int elem_bytes(int dtype) { return dtype == SLACK_BF16 ? 2 : dtype == SLACK_FP8_E4M3 ? 1 : 4; }
 
 // The first launches that use a plan wait, on the device, for its upload; every stream that reads the tables is noted
 // so that slack_plan_destroy can guard the block with an event per stream.
@@ -558,9 +562,14 @@ slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, c
   if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
   cudaEvent_t ev_after;
   if ((st = prof_begin(ctx, 1, cs, &ev_after)) != SLACK_OK) return st;
-  SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, plan->d_streams, hp.n_streams, plan->max_q_len,
-                                   plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, elem_bytes(hp.dtype),
-                                   ctx->sm_count, cs, &ctx->last_launches));
+  if (hp.dtype == SLACK_FP8_E4M3) // k_new / v_new are bf16: the append quantises (quant.cu)
+    SLACK_CUDA(ctx, launch_kv_append_fp8(k_new, v_new, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, plan->d_streams,
+                                         hp.n_streams, plan->max_q_len, plan->d_page_tables, hp.n_heads, hp.page_size, cs,
+                                         &ctx->last_launches));
+  else
+    SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, plan->d_streams, hp.n_streams, plan->max_q_len,
+                                     plan->d_page_tables, hp.n_heads, hp.head_dim, hp.page_size, elem_bytes(hp.dtype),
+                                     ctx->sm_count, cs, &ctx->last_launches));
   return prof_end(ctx, 1, cs, ev_after);
 }
 
@@ -576,7 +585,7 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
   HostPlan hp;
   std::string err;
   slack_plan_opts o{};
-  o.force_simt = 1;
+  o.force_simt = pool->dtype != SLACK_FP8_E4M3;
   try {
     st = build_plan(*pool, n_streams, streams, o, ctx->sm_count, hp, err);
   } catch (const std::bad_alloc &) {
@@ -601,7 +610,11 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
   int max_q = 0;
   for (const DevStream &s : hp.streams) max_q = s.q_len > max_q ? s.q_len : max_q;
   cudaError_t e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, cs);
-  if (e == cudaSuccess)
+  if (e == cudaSuccess && hp.dtype == SLACK_FP8_E4M3)
+    e = launch_kv_append_fp8(k_new, v_new, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, reinterpret_cast<DevStream *>(d),
+                             hp.n_streams, max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.page_size, cs,
+                             &ctx->last_launches);
+  else if (e == cudaSuccess)
     e = launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, reinterpret_cast<DevStream *>(d), hp.n_streams, max_q,
                          reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.head_dim, hp.page_size,
                          elem_bytes(hp.dtype), ctx->sm_count, cs, &ctx->last_launches);
@@ -632,6 +645,7 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
   if (!src_pools || !dst_pools || !src_page_ids || !dst_page_ids) return set_err(ctx, SLACK_EINVAL, "NULL argument");
   const slack_pool &s0 = src_pools[0];
   const slack_pool &d0 = dst_pools[0];
+  if (s0.dtype == SLACK_FP8_E4M3) return set_err(ctx, SLACK_EUNSUPPORTED, "slack_kv_transfer: FP8 pools (codes + scales) are not built");
   if (s0.n_heads <= 0 || s0.head_dim <= 0 || s0.page_size <= 0 || (s0.dtype != SLACK_BF16 && s0.dtype != SLACK_F32))
     return set_err(ctx, SLACK_EINVAL, "bad source pool shape / dtype");
   if (((size_t)s0.page_size * s0.head_dim * elem_bytes(s0.dtype)) % 16 != 0)
@@ -715,7 +729,9 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   if (!q || !out || !aligned(q, 16) || !aligned(out, 16)) return set_err(ctx, SLACK_EINVAL, "q / out NULL or not 16-byte aligned");
   if (!(scale > 0.f) || !(scale < 1e30f)) return set_err(ctx, SLACK_EINVAL, "scale must be a positive finite number");
   cudaStream_t cs = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const bool fp8 = hp.dtype == SLACK_FP8_E4M3;
   if (block_mask) {
+    if (fp8) return set_err(ctx, SLACK_EUNSUPPORTED, "block-sparse attention over an FP8 pool is not built");
     if (!aligned(block_mask, 4)) return set_err(ctx, SLACK_EINVAL, "block_mask must be 4-byte aligned");
     if (mask_words < hp.mask_words_min) return set_err(ctx, SLACK_EINVAL, "mask_words smaller than slack_plan_mask_min_words()");
     if (hp.max_item_steps > 65535)
@@ -749,10 +765,13 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   const bool pairs = hp.kernel_kind == 2 && !block_mask;
   CUtensorMap tm_q, tm_k, tm_v;
   const uint64_t pool_rows = (uint64_t)hp.n_pages * hp.n_heads * hp.page_size;
-  if ((st = make_map(ctx, &tm_q, q, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
-  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows, pairs ? 64 : 128)) != SLACK_OK) return st;
-  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows)) != SLACK_OK) return st;
+  uint8_t *q8 = fp8 ? reinterpret_cast<uint8_t *>(workspace) + hp.q8_off : nullptr; // FP8: Q is quantised into the workspace first
+  float *q8_scale = fp8 ? reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + hp.q8_scale_off) : nullptr;
+  if ((st = make_map(ctx, &tm_q, fp8 ? (const void *)q8 : q, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q, 128, fp8)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_k, pool->k_pool, (uint64_t)hp.head_dim, pool_rows, pairs ? 64 : 128, fp8)) != SLACK_OK) return st;
+  if ((st = make_map(ctx, &tm_v, pool->v_pool, (uint64_t)hp.head_dim, pool_rows, 128, fp8)) != SLACK_OK) return st;
   if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
+  if (fp8) SLACK_CUDA(ctx, launch_q_quant(q, q8, q8_scale, hp.total_q, hp.n_heads, cs, &ctx->last_launches));
   TcParams p{};
   p.items = plan->d_items;
   p.cta_begin = plan->d_cta_begin;
@@ -772,6 +791,11 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   p.page_log2 = pl2;
   p.total_q = hp.total_q;
   p.scale = scale;
+  if (fp8) {
+    p.k_scale = pool->k_scale;
+    p.v_scale = pool->v_scale;
+    p.q_scale = q8_scale;
+  }
   if (block_mask) { // the mask may change with every call: list each item's selected key-tile steps first
     uint8_t *w8 = reinterpret_cast<uint8_t *>(workspace);
     uint16_t *steps = reinterpret_cast<uint16_t *>(w8 + hp.sparse_steps_off);

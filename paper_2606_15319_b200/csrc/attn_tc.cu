@@ -20,9 +20,18 @@
 // per layer / denoising step, the host plan does not); every role walks that list instead of 0..T-1, an item with an
 // empty list writes zeros (lse = -inf) and touches no barrier.
 //
+// FP8 variant (kFp8, PAPER.md P:88 knob (4); rule in include/slack.h slack_dtype / DESIGN.md A19):
+// the pool holds e4m3 codes with one scale per (page, head, 128-slot block) = per key tile, Q arrives as e4m3 codes with one
+// scale per (row, head) (quant.cu), both MMAs are tcgen05 kind::f8f6f4 (K = 32: 4 instructions per tile instead of 8) and
+// P is rounded to e4m3 (4 codes per TMEM column).  With sq, sk_t, sv_t the scales of the row, of K tile t and of V tile t,
+//     z = S * (scale log2e sq sk_t) + log2 sv_t,     P = 128 * 2^(z - m)  (m = running max of z, lazily rescaled),
+//     O += P V8,   l += (sum_tile P) / (128 sv_t),   out = O / (128 l),   lse = (m + log2 l) ln 2
+// i.e. the V scale rides inside P's exponent and the row sum is corrected once per tile: no per-element scale work.
+//
 // Shared memory layouts (all 128-byte swizzled, as TMA writes them and as the UMMA descriptors expect them):
 //   Q tile / K tile: two 16 KB halves (d 0..63, d 64..127), each [128 rows][128 B]  -> K-major operands
 //   V tile:          same bytes; read as the MN-major B operand of P V (N = d contiguous, K = keys)
+//   FP8: every tile is ONE [128 rows][128 B] block of 16 KB (a row = the 128 codes of one token / query row)
 #include <cuda_bf16.h>
 
 #include "kernels.h"
@@ -55,11 +64,18 @@ enum : int {
   NUM_BARS = BAR_O_FREE + 2
 };
 constexpr uint32_t kOffTmemPtr = kOffBar + NUM_BARS * 8;
-constexpr uint32_t kSmemUsed = kOffTmemPtr + 16;
+constexpr int kScaleRing = 16; // FP8: scale of ring entry r (a K or a V tile) at slot r % 16; the producer runs at most
+                               // kStages entries ahead of the MMAs and the softmax at most 4 behind them
+constexpr uint32_t kOffScale = kOffTmemPtr + 16;
+constexpr uint32_t kSmemUsed = kOffScale + kScaleRing * 4;
 constexpr uint32_t kSmemBytes = kSmemUsed + 1024; // slack for manual 1024-byte alignment
 
 constexpr uint32_t kIdescQK = make_idesc_bf16(128, 128, 0, 0);
 constexpr uint32_t kIdescPV = make_idesc_bf16(128, 128, 0, 1);
+constexpr uint32_t kIdescQK8 = make_idesc_e4m3(128, 128, 0, 0);
+constexpr uint32_t kIdescPV8 = make_idesc_e4m3(128, 128, 0, 1);
+constexpr uint32_t kTileBytes8 = 16384;
+constexpr float kRescaleThreshold8 = 1.0f; // FP8: P = 128 * 2^(z - m) must stay below e4m3's 448
 
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -118,7 +134,7 @@ __device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
       p.dbg_t[((role) * 64 + (step)) * 8 + (slot)] = (uint32_t)clock64();                                  \
   }
 
-template <bool kTrace, bool kSparse>
+template <bool kTrace, bool kSparse, bool kFp8>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                const __grid_constant__ CUtensorMap tm_v) {
@@ -128,6 +144,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
   const uint32_t sKV = smem_base + kOffKV;
   const uint32_t bars = smem_base + kOffBar;
   const uint32_t tmem_ptr_smem = smem_base + kOffTmemPtr;
+  const uint32_t sScale = smem_base + kOffScale;
   auto bar = [&](int i) { return bars + 8u * (uint32_t)i; };
 
   // warp-uniform by construction, and provably so for the compiler (keeps the role branches and everything the
@@ -199,34 +216,52 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
         ++n_item;
         if (elect_one()) {
-          mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes);
-          for (int i = 0; i < v.nq; ++i)
-            for (int c = 0; c < 2; ++c)
-              tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), head * 128 + c * 64,
-                          q_row0 + i * kTileM);
+          if constexpr (kFp8) { // one [128 rows][128 codes] box per query tile
+            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes8);
+            for (int i = 0; i < v.nq; ++i) tma_load_2d(sQ + i * kTileBytes, &tm_q, bar(BAR_Q_FULL), head * 128, q_row0 + i * kTileM);
+          } else {
+            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes);
+            for (int i = 0; i < v.nq; ++i)
+              for (int c = 0; c < 2; ++c)
+                tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), head * 128 + c * 64,
+                            q_row0 + i * kTileM);
+          }
         }
         __syncwarp();
         for (int j0 = 0; j0 < Ts; j0 += 32) { // 32 steps at a time: each lane looks up the pool row of one step's tile
           const int my_jj = j0 + lane;
           int my_row = 0;
+          float my_sk = 1.f, my_sv = 1.f;
           if (my_jj < Ts) {
             const int my_tile = v.tile_of(kSparse ? (int)__ldg(steps + my_jj) : my_jj);
             const int my_page = __ldg(p.page_tables + pt_off + ((my_tile * kTileN) >> p.page_log2));
             my_row = (my_page * H + head) * P + ((my_tile * kTileN) & (P - 1));
+            if constexpr (kFp8) { // the tile's scales: one per (page, head, 128-slot block)
+              const size_t si = ((size_t)my_page * H + head) * (size_t)(P >> 7) + (size_t)(((my_tile * kTileN) & (P - 1)) >> 7);
+              my_sk = __ldg(p.k_scale + si);
+              my_sv = __ldg(p.v_scale + si);
+            }
           }
           const int cnt = min(32, Ts - j0);
           for (int j = 0; j < cnt; ++j) {
             const int row = __shfl_sync(0xffffffffu, my_row, j);
+            [[maybe_unused]] const float t_sk = __shfl_sync(0xffffffffu, my_sk, j), t_sv = __shfl_sync(0xffffffffu, my_sv, j);
 #pragma unroll
             for (int kv = 0; kv < 2; ++kv) {
               const uint32_t stage = ring % kStages;
               const uint32_t ph = (ring / kStages) & 1u;
               mbar_wait(bar(BAR_KV_EMPTY + stage), ph ^ 1u, 110 + stage, dbg);
               if (elect_one()) {
-                mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes);
                 const CUtensorMap *tm = kv == 0 ? &tm_k : &tm_v;
-                tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
-                tma_load_2d(sKV + stage * kTileBytes + kHalfBytes, tm, bar(BAR_KV_FULL + stage), 64, row);
+                if constexpr (kFp8) {
+                  st_shared_f32(sScale + (ring % kScaleRing) * 4u, kv == 0 ? t_sk : t_sv); // read by the softmax warps
+                  mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes8);
+                  tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
+                } else {
+                  mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes);
+                  tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
+                  tma_load_2d(sKV + stage * kTileBytes + kHalfBytes, tm, bar(BAR_KV_FULL + stage), 64, row);
+                }
               }
               __syncwarp();
               ++ring;
@@ -244,11 +279,18 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         const uint32_t a_base = sQ + i * kTileBytes;
         const uint32_t b_base = sKV + stage * kTileBytes;
         const uint32_t d = tmem_base + (uint32_t)(i * 128);
+        if constexpr (kFp8) { // K = 32 codes = 32 bytes per instruction, the whole head_dim in one 128-byte row
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          const uint32_t off = (uint32_t)(k >> 2) * kHalfBytes + (uint32_t)(k & 3) * 32u;
-          mma_ss(d, make_smem_desc_sw128(a_base + off, 16, 1024), make_smem_desc_sw128(b_base + off, 16, 1024), kIdescQK,
-                 k > 0 ? 1u : 0u);
+          for (int k = 0; k < 4; ++k)
+            mma_ss_f8(d, make_smem_desc_sw128(a_base + (uint32_t)k * 32u, 16, 1024), make_smem_desc_sw128(b_base + (uint32_t)k * 32u, 16, 1024),
+                      kIdescQK8, k > 0 ? 1u : 0u);
+        } else {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const uint32_t off = (uint32_t)(k >> 2) * kHalfBytes + (uint32_t)(k & 3) * 32u;
+            mma_ss(d, make_smem_desc_sw128(a_base + off, 16, 1024), make_smem_desc_sw128(b_base + off, 16, 1024), kIdescQK,
+                   k > 0 ? 1u : 0u);
+          }
         }
       };
       // P V over keys [64*half, 64*half + 64) of the tile (4 MMAs of K = 16)
@@ -256,11 +298,20 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         const uint32_t b_base = sKV + stage * kTileBytes;
         const uint32_t d = tmem_base + (uint32_t)(256 + i * 128);
         const uint32_t a = tmem_base + (uint32_t)(i * 128);
+        if constexpr (kFp8) { // 2 instructions of K = 32 keys (8 TMEM columns of P, 32 rows x 128 B of V) per half
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) {
-          const int k = half * 4 + kk;
-          mma_ts(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 2048u, kHalfBytes, 1024), kIdescPV,
-                 (acc || k > 0) ? 1u : 0u);
+          for (int kk = 0; kk < 2; ++kk) {
+            const int k = half * 2 + kk;
+            mma_ts_f8(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 4096u, kHalfBytes, 1024), kIdescPV8,
+                      (acc || k > 0) ? 1u : 0u);
+          }
+        } else {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk) {
+            const int k = half * 4 + kk;
+            mma_ts(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 2048u, kHalfBytes, 1024), kIdescPV,
+                   (acc || k > 0) ? 1u : 0u);
+          }
         }
       };
       for (int k = item_begin; k < item_end; ++k) {
@@ -308,10 +359,11 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             if (c_lo > 0 || c_hi < kTileN) {
               const int n_zero = c_lo + (kTileN - c_hi);
               const uint32_t base = sKV + stage_v * kTileBytes;
-              for (int idx = lane; idx < n_zero * 16; idx += 32) {
-                int r = idx >> 4;
+              constexpr int kVecs = kFp8 ? 8 : 16; // 16-byte vectors per key row (FP8: one 128-byte row; bf16: two)
+              for (int idx = lane; idx < n_zero * kVecs; idx += 32) {
+                int r = idx / kVecs;
                 r = r < c_lo ? r : c_hi + (r - c_lo);
-                const int w = idx & 15;
+                const int w = idx % kVecs;
                 const uint32_t addr = base + (uint32_t)(w >> 3) * kHalfBytes + (uint32_t)r * 128u + (uint32_t)(w & 7) * 16u;
                 asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
               }
@@ -364,10 +416,13 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
     const uint32_t tO = tmem_base + lane_addr + (uint32_t)(256 + i * 128);
     const float sl2 = p.scale * kLog2e;
     uint32_t cnt = 0, itn = 0;
+    [[maybe_unused]] uint32_t ring = 0; // FP8: ring entry of the item's first K tile (the producer's count; scale slots)
     bool first_item = true;
     for (int k = item_begin; k < item_end; ++k) {
       const DevItem it = p.items[k];
       const ItemView v = view_of(it);
+      [[maybe_unused]] const uint32_t r0 = ring;
+      if constexpr (kFp8) ring += 2u * (uint32_t)v.T; // every role counts the item's tiles, also the one that skips it
       if (i >= v.nq) continue;
       const int Ts = kSparse ? p.item_steps[k] : v.T;
       const uint16_t *steps = kSparse ? p.steps + it.step_off : nullptr;
@@ -390,6 +445,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         continue;
       }
       float m = -INFINITY, l = 0.f;
+      // FP8: scale of this thread's query row (rows past the end of Q hold garbage that is never stored)
+      [[maybe_unused]] float q_sc = 1.f;
+      if constexpr (kFp8) q_sc = __ldg(p.q_scale + (size_t)it.head * p.total_q + min(it.q_row0 + i * kTileM + row, p.total_q - 1));
       int j_dense = kSparse ? (int)__ldg(steps) : 0;
       for (int j = 0; j < Ts; ++j) {
         const int jd = j_dense; // dense step index (block-sparse: the next one is fetched a step ahead)
@@ -437,14 +495,28 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           for (int c = 0; c < 4; ++c) mxc[c] = fmaxf(mxc[c], s[c * 32 + 31]);
           return fmaxf(max3(mxc[0], mxc[1], mxc[2]), mxc[3]);
         };
-        if (j == 0) m = row_max();
+        // logit -> exponent: z = s * cz + az.  bf16: cz = scale log2e, az = 0 and m is kept in units of s (z = s cz).
+        // FP8: cz = scale log2e sq sk_t, az = log2 sv_t (the V scale rides inside P), m is kept in units of z, and P is
+        // scaled by 2^7 so that its e4m3 codes use the range up to 128 (x 2 before a lazy rescale) of the format's 448.
+        float cz = sl2, az = 0.f, l_fix = 1.f;
+        if constexpr (kFp8) {
+          const float t_sk = ld_shared_f32(sScale + ((r0 + 2u * (uint32_t)j) % kScaleRing) * 4u);
+          const float t_sv = ld_shared_f32(sScale + ((r0 + 2u * (uint32_t)j + 1u) % kScaleRing) * 4u);
+          cz = sl2 * q_sc * t_sk;
+          az = log2f(t_sv);
+          l_fix = 0.0078125f / t_sv; // this tile's P sums, taken in units of 128 sv_t, back to plain probabilities
+        }
+        auto to_m = [&](float mx_s) { return kFp8 ? fmaf(mx_s, cz, az) : mx_s; };       // row max of s -> units of m
+        auto neg_m = [&]() { return kFp8 ? (az - m + 7.0f) : (-m * sl2); };               // addend of the exponent
+        constexpr float kThr = kFp8 ? kRescaleThreshold8 : kRescaleThreshold;
+        if (j == 0) m = to_m(row_max());
         SLACK_TRACE(i, j, 3);
-        // P = 2^(s*sl2 - m*sl2) on packed pairs: FFMA2 for the argument, then either 2 MUFU.EX2 or (kEmuOf8 pairs out
-        // of every 8) the FMA-pipe polynomial; FADD2 row sums; one F2FP per pair.
-        const uint64_t sl2_2 = pack2(sl2, sl2);
-        uint64_t negm_2 = pack2(-m * sl2, -m * sl2);
+        // P = 2^(s*cz + addend) on packed pairs: FFMA2 for the argument, then either 2 MUFU.EX2 or (kEmuOf8 pairs out
+        // of every 8) the FMA-pipe polynomial; FADD2 row sums; one F2FP per pair (FP8: per four).
+        const uint64_t sl2_2 = pack2(cz, cz);
+        uint64_t negm_2 = pack2(neg_m(), neg_m());
         uint64_t la0 = pack2(0.f, 0.f), la1 = la0;
-        auto exp_chunk = [&](int c) { // 32 columns -> 16 packed bf16x2 columns of P
+        auto exp_chunk = [&](int c) { // 32 columns -> 16 packed bf16x2 (FP8: 8 packed e4m3x4) columns of P
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 16; ++e) {
@@ -460,18 +532,37 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             if (e & 1) la1 = fadd2(la1, p2); else la0 = fadd2(la0, p2);
             float p0, p1;
             unpack2(p2, p0, p1);
-            pk[e] = pack_bf16x2(p0, p1);
+            if constexpr (kFp8) { // two pairs -> one column of four e4m3 codes
+              if (e & 1) pk[e >> 1] = pack_e4m3x4(__uint_as_float(pk[e >> 1]), __uint_as_float(pk[8 + (e >> 1)]), p0, p1);
+              else pk[e >> 1] = __float_as_uint(p0), pk[8 + (e >> 1)] = __float_as_uint(p1);
+            } else {
+              pk[e] = pack_bf16x2(p0, p1);
+            }
           }
-          tmem_st16(tS + (uint32_t)(c * 16), pk);
+          if constexpr (kFp8) {
+            uint32_t p8[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) p8[e] = pk[e];
+            tmem_st8(tS + (uint32_t)(c * 8), p8);
+          } else {
+            tmem_st16(tS + (uint32_t)(c * 16), pk);
+          }
+        };
+        // the row sums collected since the last call, into l (FP8: in this tile's units of 128 sv_t)
+        auto flush_sums = [&]() {
+          float a0, a1;
+          unpack2(fadd2(la0, la1), a0, a1);
+          l = fmaf(a0 + a1, l_fix, l);
         };
         {
-          const float mx = row_max(); // independent of the two chunks below: the scheduler interleaves them
+          const float mx = to_m(row_max()); // independent of the two chunks below: the scheduler interleaves them
           exp_chunk(0);
           exp_chunk(1);
-          const bool need = (mx - m) * sl2 > kRescaleThreshold; // never on the first tile (m == mx)
+          const float grow = kFp8 ? (mx - m) : (mx - m) * sl2;
+          const bool need = grow > kThr; // never on the first tile (m == mx)
           if (__any_sync(0xffffffffu, need)) {
             // PV of the previous key tile has completed (its commit precedes S_FULL in the in-order tensor pipe)
-            const float alpha = need ? ex2((m - mx) * sl2) : 1.0f;
+            const float alpha = need ? ex2(-grow) : 1.0f;
             m = need ? mx : m;
             l *= alpha;
 #pragma unroll
@@ -483,7 +574,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
               for (int e = 0; e < 32; ++e) r[e] = __float_as_uint(__uint_as_float(r[e]) * alpha);
               tmem_st32(tO + (uint32_t)(c * 32), r);
             }
-            negm_2 = pack2(-m * sl2, -m * sl2);
+            negm_2 = pack2(neg_m(), neg_m());
             la0 = la1 = pack2(0.f, 0.f);
             exp_chunk(0);
             exp_chunk(1);
@@ -496,11 +587,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         if (lane == 0) mbar_arrive(bar(BAR_P_LO + i)); // P V over keys 0..63 may start
         exp_chunk(2);
         exp_chunk(3);
-        {
-          float a0, a1;
-          unpack2(fadd2(la0, la1), a0, a1);
-          l += a0 + a1;
-        }
+        flush_sums();
         SLACK_TRACE(i, j, 5);
         tmem_wait_st();
         tc_fence_before();
@@ -515,10 +602,10 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       // ---------------- epilogue: O / l ----------------
       mbar_wait(bar(BAR_O_FINAL + i), itn & 1u, 310 + i, dbg);
       tc_fence_after();
-      const float inv_l = 1.0f / l;
+      const float inv_l = kFp8 ? 0.0078125f / l : 1.0f / l; // FP8: O was accumulated from P = 128 * probabilities
       const int local_row = i * kTileM + row;
       const bool valid = local_row < it.q_rows;
-      const float lse_val = (m * sl2 + log2f(l)) * kLn2;
+      const float lse_val = ((kFp8 ? m : m * sl2) + log2f(l)) * kLn2;
       if (it.partial_slot < 0) {
         __nv_bfloat16 *dst =
             reinterpret_cast<__nv_bfloat16 *>(p.out) + ((size_t)(it.q_row0 + local_row) * H + it.head) * 128;
@@ -589,27 +676,33 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 size_t attn_tc_smem_bytes() { return kSmemBytes; }
 
 cudaError_t attn_tc_configure() {
-  cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(attn_tc_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
 #ifdef SLACK_DIAGNOSTICS
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(attn_tc_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  e = cudaFuncSetAttribute(attn_tc_kernel<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
 #endif
   return e;
 }
 
+// p.q_scale != null selects the FP8 instantiation (tm_q / tm_k / tm_v are then byte maps with [128 x 128 B] boxes);
+// p.steps != null the block-sparse one
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched) {
   cudaError_t e;
-  if (p.steps != nullptr)
-    e = launch_pdl(attn_tc_kernel<false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+  if (p.q_scale != nullptr)
+    e = launch_pdl(attn_tc_kernel<false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+  else if (p.steps != nullptr)
+    e = launch_pdl(attn_tc_kernel<false, true, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
 #ifdef SLACK_DIAGNOSTICS
   else if (p.dbg_t != nullptr || p.dbg_s != nullptr)
-    e = launch_pdl(attn_tc_kernel<true, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+    e = launch_pdl(attn_tc_kernel<true, false, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
 #endif
   else
-    e = launch_pdl(attn_tc_kernel<false, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+    e = launch_pdl(attn_tc_kernel<false, false, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   if (n_launched) *n_launched += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -60,6 +60,9 @@ struct TcParams {
   unsigned long long *dbg_flag; // 4-word host-mapped record a timed-out barrier wait fills before it traps
   const uint16_t *steps;        // block-sparse: compacted step lists (sparse_steps.cu), else null = dense
   const int32_t *item_steps;    // block-sparse: selected steps per item
+  const float *k_scale;         // FP8 pools: [n_pages][H][P / 128] scales of the K / V codes, else null
+  const float *v_scale;
+  const float *q_scale;         // FP8 pools: [H][total_q] scales of the quantised Q (q_quant_kernel)
   int32_t n_heads;
   int32_t page_log2;
   int32_t total_q;
@@ -69,6 +72,12 @@ size_t attn_tc_smem_bytes();
 cudaError_t attn_tc_configure(); // cudaFuncSetAttribute(max dynamic smem); once per process/device
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched);
+
+// NEXT-3 (quant.cu): quantising append into an FP8 pool, and the Q quantiser of the FP8 attention call.
+cudaError_t launch_kv_append_fp8(const void *k_new, const void *v_new, void *k_pool, void *v_pool, float *k_scale, float *v_scale,
+                                 const DevStream *d_streams, int n_streams, int max_q_len, const int32_t *d_page_tables,
+                                 int n_heads, int page_size, cudaStream_t st, int *n_launched);
+cudaError_t launch_q_quant(const void *q, void *q8, float *sq, int total_q, int n_heads, cudaStream_t st, int *n_launched);
 
 // A3 on CTA pairs (attn_tc2.cu, tcgen05 cta_group::2): needs a pair plan (HostPlan::kernel_kind 2, even n_cta) and a K
 // tensor map with 64-row boxes (each CTA loads half of a key tile's keys).

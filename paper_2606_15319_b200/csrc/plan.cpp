@@ -260,7 +260,8 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   };
   if (n_streams < 0 || (n_streams > 0 && !streams)) return fail(SLACK_EINVAL, "n_streams < 0 or streams == NULL");
   if (shape.n_pages <= 0 || shape.n_heads <= 0) return fail(SLACK_EINVAL, "pool: n_pages and n_heads must be > 0");
-  if (shape.dtype != SLACK_BF16 && shape.dtype != SLACK_F32) return fail(SLACK_EINVAL, "pool: unknown dtype");
+  if (shape.dtype != SLACK_BF16 && shape.dtype != SLACK_F32 && shape.dtype != SLACK_FP8_E4M3)
+    return fail(SLACK_EINVAL, "pool: unknown dtype");
   if (shape.head_dim != 64 && shape.head_dim != 128) return fail(SLACK_EUNSUPPORTED, "head_dim must be 64 or 128");
   if (!is_pow2(shape.page_size) || shape.page_size < 16)
     return fail(SLACK_EUNSUPPORTED, "page_size must be a power of two >= 16");
@@ -274,7 +275,10 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   out.dtype = shape.dtype;
   out.n_streams = n_streams;
   out.n_cta = opts.sm_count > 0 ? opts.sm_count : default_sm_count;
-  const bool tc_ok = shape.dtype == SLACK_BF16 && shape.head_dim == 128 && shape.page_size >= kTileN;
+  const bool fp8 = shape.dtype == SLACK_FP8_E4M3;
+  if (fp8 && (shape.head_dim != 128 || shape.page_size < kTileN || opts.force_simt))
+    return fail(SLACK_EUNSUPPORTED, "FP8 pools need head_dim 128, page_size >= 128 and the tensor-core kernel");
+  const bool tc_ok = (shape.dtype == SLACK_BF16 || fp8) && shape.head_dim == 128 && shape.page_size >= kTileN;
   if (opts.cta_pairs < 0 || opts.cta_pairs > 2) return fail(SLACK_EINVAL, "plan opts: cta_pairs must be 0, 1 or 2");
   out.kernel_kind = (tc_ok && !opts.force_simt) ? 0 : 1;
 
@@ -332,6 +336,13 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     d.pos_hi = (int32_t)end_pos;
     d.sink_hi = (int32_t)(s.base + (one_range ? 0 : sink));
     d.app_pos0 = (int32_t)(s.base + s.cache_len + (s.cache_len >= s.sink_len ? s.gap_slots : 0));
+    if (s.gap_slots > 0) { // earlier tokens: the sink [base, base + sink) and, behind the hole, [base + gap + sink, app_pos0)
+      d.old_hi0 = s.base + s.sink_len;
+      d.old_lo1 = s.base + s.gap_slots + s.sink_len;
+    } else {
+      d.old_hi0 = s.base + s.cache_len;
+      d.old_lo1 = d.app_pos0;
+    }
     d.pt_off = (int32_t)out.page_tables.size();
     d.n_table_pages = need;
     for (int32_t p = 0; p < need; ++p) {
@@ -379,7 +390,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   // the even CTA and the rest on the odd one, and share every K/V tile.  The plan is then made for n_cta / 2 queues.
   // Pays when most items have more than 128 rows; short chunks (decode-like) keep one CTA per item.
   // cta_pairs: 0 = automatic, 1 = never, 2 = always (needs an even CTA count).
-  if (out.n_cta >= 2 && out.n_cta % 2 == 0) {
+  if (out.n_cta >= 2 && out.n_cta % 2 == 0 && !fp8) {
     bool pairs = opts.cta_pairs == 2;
     if (opts.cta_pairs == 0 && kAutoPairs) {
       int64_t rows = 0, padded = 0;
@@ -449,6 +460,11 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   out.ws.o_bytes = (size_t)out.n_partial_slots * kItemRows * shape.head_dim * sizeof(float);
   out.ws.lse_off = out.ws.o_bytes;
   out.ws.total = out.ws.o_bytes + (size_t)out.n_partial_slots * kItemRows * sizeof(float);
+  if (fp8) { // room for the quantised Q behind the split-KV partials
+    out.q8_off = (out.ws.total + 127) & ~(size_t)127;
+    out.q8_scale_off = out.q8_off + (size_t)out.total_q * shape.n_heads * shape.head_dim;
+    out.ws.total = out.q8_scale_off + (size_t)out.total_q * shape.n_heads * sizeof(float);
+  }
   // block-sparse bookkeeping: which mask row an item reads and where its compacted step list goes
   for (DevItem &it : out.items) {
     const DevStream &d = out.streams[it.stream];

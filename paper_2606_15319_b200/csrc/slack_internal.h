@@ -63,9 +63,11 @@ struct DevStream {
   int32_t sink_hi;  // visible sink positions [base, sink_hi) in front of [pos_lo, pos_hi); == base when there are none
   int32_t qblock0;  // global index of the stream's first 256-row query block (row of the block mask)
   int32_t app_pos0; // position of the first token the append writes: pos(cache_len) (slack.h token -> slot rule)
-  int32_t pad;
+  int32_t old_hi0;  // positions of the stream's EARLIER tokens [0, cache_len): [base, old_hi0) and [old_lo1, app_pos0)
+  int32_t old_lo1;  //   (the second range is empty unless a hole sits behind the sink; FP8 append: who owns a scale block)
+  int32_t pad[3];
 };
-static_assert(sizeof(DevStream) == 48, "DevStream layout");
+static_assert(sizeof(DevStream) == 64, "DevStream layout");
 
 // Workspace layout for split-KV partials: slot s holds kItemRows rows of head_dim fp32 (normalised partial output)
 // followed, in a second region, by kItemRows fp32 lse values.
@@ -90,6 +92,8 @@ struct HostPlan {
   std::vector<DevCombine> combines;
   int32_t n_partial_slots = 0;
   WorkspaceLayout ws;
+  // FP8 pools: the attention call quantises Q into the workspace first: codes [total_q][H][128] u8, scales [H][total_q] f32
+  size_t q8_off = 0, q8_scale_off = 0;
   // block-sparse variant (slack_chunk_attention_sparse): mask geometry and the extra workspace behind ws.total
   int32_t mask_rows = 0;        // sum over streams of ceil(q_len / 256)
   int32_t mask_words_min = 1;   // 32-bit words a mask row needs: ceil(max_s ceil(pos_hi / 128) / 32)

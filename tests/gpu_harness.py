@@ -105,3 +105,16 @@ def check_attention(w, out_np, lse_np, want, want_lse, max_abs_tol=2e-2, rel_fro
             res["lse_max_abs"] = le
             assert le <= lse_tol, f"{w.name}: lse max_abs {le:.3e}"
     return res
+
+
+# ---------------------------------------------------------------------------------------------------- FP8 pools (NEXT-3)
+def make_pool_fp8(w, device="cuda:0", code_fill=0x7F, scale_fill=float("nan")):
+    """e4m3 code pools filled with the NaN code and scales filled with NaN: whatever the append does not write stays put."""
+    shape = (w.n_pages, w.n_heads, w.page_size, w.head_dim)
+    k = torch.full(shape, code_fill, dtype=torch.uint8, device=device)
+    ks = torch.full((w.n_pages, w.n_heads, w.page_size // 128), scale_fill, dtype=torch.float32, device=device)
+    return binding.Pool(k, k.clone(), w.n_pages, w.n_heads, w.head_dim, w.page_size, "fp8", k_scale=ks, v_scale=ks.clone())
+
+
+def fp8_pool_images(pool):
+    return (pool.k_pool.cpu().numpy(), pool.v_pool.cpu().numpy(), pool.k_scale.cpu().numpy(), pool.v_scale.cpu().numpy())

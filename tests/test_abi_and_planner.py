@@ -38,7 +38,7 @@ def test_every_declared_symbol_is_exported_and_bound():
         assert n in exported, f"{n} declared in slack.h but not exported"
         assert n in binding.SYMBOLS, f"{n} has no ctypes signature in the binding"
     lib = binding.load()
-    assert lib.slack_abi_version() == 2
+    assert lib.slack_abi_version() == 3
     # include/slack_diag.h is exported by -DSLACK_DIAGNOSTICS builds only; the default library carries none of it
     assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["slack.h", "slack_diag.h"]
     diag = declared_symbols("slack_diag.h")
@@ -51,7 +51,7 @@ def test_every_declared_symbol_is_exported_and_bound():
 
 def test_struct_sizes_match_header():
     import ctypes as C
-    assert C.sizeof(binding.CPool) == 40 and C.sizeof(binding.CStream) == 40
+    assert C.sizeof(binding.CPool) == 56 and C.sizeof(binding.CStream) == 40
     assert C.sizeof(binding.CPlanOpts) == 16 and C.sizeof(binding.CWorkItem) == 48
 
 

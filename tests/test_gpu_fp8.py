@@ -1,0 +1,162 @@
+"""-m gpu parity tests of the FP8 path (PAPER.md P:88 knob (4); rule: include/slack.h slack_dtype,
+DESIGN.md A19), through the C ABI against oracle/fp8_attention.py on the same seeded inputs.
+
+* the quantising append is BIT-EXACT: every code and every scale of the whole pool image, untouched bytes included;
+* attention is compared with the oracle's definition on the DEQUANTISED Q, K, V (exact P).  The kernel additionally rounds
+  P to e4m3 (3 mantissa bits: relative error up to 2^-4, ~2.6 % rms); with the i.i.d. zero-mean V of the synthetic
+  workloads that error does not average out RELATIVE to the output (signal and noise both shrink like 1/sqrt(keys)), so the
+  gate is rel-Fro <= 4e-2 and max-abs <= 2e-2 (A19 derives it); inputs whose V has a common component are held
+  to 5e-3, which is what catches a wrong scale, exponent offset or normalisation."""
+import copy
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import fp8_attention as F
+from paper_2606_15319_b200 import binding, workloads as W
+import gpu_harness as G
+from helpers import oracle_pools_fp8
+
+pytestmark = pytest.mark.gpu
+TOL = dict(max_abs_tol=2e-2, rel_fro_tol=4e-2, lse_tol=2e-2)
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device; the product has no CPU fallback"
+    c = binding.Context(0)
+    yield c
+    c.close()
+
+
+def assert_pool_equals_oracle(w, pool):
+    kc, vc, ks, vs = oracle_pools_fp8(w)
+    gk, gv, gks, gvs = G.fp8_pool_images(pool)
+    assert np.array_equal(gks, ks, equal_nan=True) and np.array_equal(gvs, vs, equal_nan=True), "scales differ"
+    assert np.array_equal(gk, kc) and np.array_equal(gv, vc), "codes differ"
+
+
+@pytest.mark.parametrize("make", [W.small_ragged, lambda: W.small_ragged(page_size=256), W.sink_ragged, W.gap_ragged,
+                                  lambda: W.small_ragged(page_size=512, seed=5)])
+def test_quantising_append_bit_exact(ctx, make):
+    w = make()
+    pool = G.make_pool_fp8(w)
+    G.gpu_append_all(ctx, w, pool)
+    assert_pool_equals_oracle(w, pool)
+
+
+def test_append_planned_reappend_and_large_values(ctx):
+    """The planned variant writes the same bytes; a later denoising step re-appends other values at the same positions
+    (blocks the chunk started get new scales, a block it continues keeps the old one and saturates: 30 x larger values)."""
+    w = W.small_ragged()
+    pool = G.make_pool_fp8(w)
+    plan = ctx.slack_plan(pool, w.streams)
+    G.gpu_append_all(ctx, w, pool, planned_plan=plan)
+    assert_pool_equals_oracle(w, pool)
+    w2 = copy.copy(w)
+    big = oracle.to_f64(w.v_new, "bf16").astype(np.float32) * np.float32(30)
+    w2.k_new, w2.v_new = W.f32_to_bf16_bits(big), w.k_new
+    ctx.slack_kv_append_planned(plan, pool, binding.to_torch(w2.k_new, "bf16", "cuda:0"), binding.to_torch(w2.v_new, "bf16", "cuda:0"))
+    torch.cuda.synchronize()
+    assert_pool_equals_oracle(w2, pool)
+    assert np.isin(G.fp8_pool_images(pool)[0], (0x7E, 0xFE)).any(), "the case must exercise saturation"
+
+
+def test_append_cfg2_full_size_bit_exact(ctx):
+    w = W.config2()
+    pool = G.make_pool_fp8(w)
+    G.gpu_append_all(ctx, w, pool)
+    assert_pool_equals_oracle(w, pool)
+
+
+def run_fp8(ctx, w, tol=TOL, rows=None, **opts):
+    pool = G.make_pool_fp8(w)
+    G.gpu_append_all(ctx, w, pool)
+    out, lse, plan, launches = G.gpu_attention(ctx, w, pool, **opts)
+    kc, vc, ks, vs = oracle_pools_fp8(w)
+    want, want_lse = F.chunk_attention_fp8(kc, vc, ks, vs, w.streams, w.q, w.scale, w.dtype, rows=rows)
+    res = G.check_attention(w, out, lse, want, want_lse, **tol)
+    if rows is None:
+        assert np.isfinite(out).all(), f"{w.name}: unwritten / non-finite output rows"
+    res.update(kind=plan.kernel_kind, slots=plan.num_partial_slots, launches=launches)
+    return res, out, want
+
+
+@pytest.mark.parametrize("page_size", [128, 256])
+@pytest.mark.parametrize("splits", [0, 1, 3])
+def test_small_ragged_fp8(ctx, page_size, splits):
+    res, *_ = run_fp8(ctx, W.small_ragged(page_size=page_size), force_splits=splits)
+    assert res["kind"] == 0 and res["launches"] >= 2          # Q quantiser + attention (+ combine)
+
+
+@pytest.mark.parametrize("make", [W.sink_ragged, W.gap_ragged])
+def test_sink_and_gap_fp8(ctx, make):
+    run_fp8(ctx, make(), force_splits=2)
+
+
+def test_common_component_in_v_is_held_to_half_a_percent(ctx):
+    """V = 100 + noise: P's rounding errors average out against the common component, so a wrong V scale, exponent offset
+    (the 2^7 shift, log2 sv) or normalisation (1 / (128 l)) shows at the 1e-3 level."""
+    w = W.small_ragged(seed=21)
+    shift = lambda a: W.f32_to_bf16_bits(oracle.to_f64(a, "bf16").astype(np.float32) + np.float32(100))
+    w.v_new = shift(w.v_new)
+    w.v_prior = [shift(v) for v in w.v_prior]
+    res, out, want = run_fp8(ctx, w, tol=dict(max_abs_tol=1.0, rel_fro_tol=5e-3, lse_tol=2e-2))
+    assert abs(np.nanmean(out) - np.nanmean(want)) < 0.2
+
+
+def test_tile_scales_differ_by_orders_of_magnitude(ctx):
+    """Chunks whose K and V magnitudes differ 64 x between key tiles: the per-tile K scale enters the logits, the per-tile V
+    scale rides in P's exponent and the row sum is corrected per tile (attn_tc.cu header): any slip shows immediately."""
+    w = W.small_ragged(seed=22)
+    for arrs in (w.k_prior, w.v_prior):
+        for i, a in enumerate(arrs):
+            x = oracle.to_f64(a, "bf16").astype(np.float32)
+            blk = (np.arange(x.shape[0]) // 128) % 3
+            x *= np.where(blk == 0, 1.0, np.where(blk == 1, 8.0, 0.125)).astype(np.float32)[:, None, None]
+            arrs[i] = W.f32_to_bf16_bits(x)
+    big = dict(TOL, max_abs_tol=0.3)              # outputs reach +-3 here (V x 8): the absolute gate scales with them
+    run_fp8(ctx, w, tol=big)
+    run_fp8(ctx, w, tol=big, force_splits=3)
+
+
+def test_adversarial_logits_fp8(ctx):
+    """Q x 8 (peaky rows) and a late +30 logit jump: the lazy rescale (threshold 2^1 here) and P's saturation bound."""
+    w = W.small_ragged(seed=23)
+    w.q = W.f32_to_bf16_bits(oracle.to_f64(w.q, "bf16").astype(np.float32) * np.float32(8))
+    # a row that rests on two or three keys is off by up to 2^-4 of a single p * v (|v| up to ~2 here): the absolute gate
+    # is widened to 8e-2 for the peaky cases, rel-Fro stays (measured 4.5e-3)
+    peaky = dict(TOL, max_abs_tol=8e-2)
+    run_fp8(ctx, w, tol=peaky)
+    w = W.small_ragged(seed=24)
+    kp = oracle.to_f64(w.k_prior[0], "bf16").astype(np.float32)
+    qd = oracle.to_f64(w.q, "bf16").astype(np.float32)
+    kp[-3:] = qd[0:3] * np.float32(40.0)          # three late keys aligned with three queries: logits far above the rest
+    w.k_prior[0] = W.f32_to_bf16_bits(kp)
+    run_fp8(ctx, w, tol=peaky)
+
+
+def test_cfg2_full_size_fp8_sampled_rows(ctx):
+    w = W.config2()
+    rng = np.random.default_rng(7)
+    rows = [np.sort(np.unique(np.concatenate([[0, 127, 128, 4607, 4608, 4679], rng.choice(s.q_len, 90, replace=False)]))) for s in w.streams]
+    res, out, want = run_fp8(ctx, w, rows=rows)
+    assert np.isfinite(out).all()
+
+
+def test_unsupported_combinations(ctx):
+    w = W.small_ragged()
+    pool = G.make_pool_fp8(w)
+    with pytest.raises(binding.SlackError) as e:
+        ctx.slack_plan(pool, w.streams, force_simt=1)
+    assert e.value.status == binding.SLACK_EUNSUPPORTED
+    w64 = W.small_ragged(page_size=64)
+    with pytest.raises(binding.SlackError) as e:
+        ctx.slack_plan(binding.Pool.shape_only(w64.n_pages, w64.n_heads, w64.head_dim, 64, "fp8"), w64.streams)
+    assert e.value.status == binding.SLACK_EUNSUPPORTED
+    bad = binding.Pool(pool.k_pool, pool.v_pool, w.n_pages, w.n_heads, w.head_dim, w.page_size, "fp8")      # no scales
+    with pytest.raises(binding.SlackError) as e:
+        ctx.slack_kv_append(bad, w.streams, binding.to_torch(w.k_new, "bf16", "cuda:0"), binding.to_torch(w.v_new, "bf16", "cuda:0"))
+    assert e.value.status == binding.SLACK_EINVAL
