@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="cfg5", choices=["cfg2", "cfg3", "cfg4", "cfg5", "cfg5b"])
     ap.add_argument("--no-others", action="store_true", help="skip the supplementary blocks under config.others")
+    ap.add_argument("--dtype", default="bf16", choices=["bf16", "fp8"],
+                    help="fp8: FP8 (e4m3) K/V pools, quantising append, FP8 attention (NEXT-3; never the headline line)")
     ap.add_argument("--kv-chunks", type=int, default=7, help="cfg5: visible chunks (1..7)")
     ap.add_argument("--layers", type=int, default=30)
     ap.add_argument("--force-splits", type=int, default=0)
@@ -288,14 +290,27 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
     gen = torch.Generator(device=dev)
     gen.manual_seed(777 + rank)
     rnd = lambda *shape: (torch.randn(*shape, device=dev, dtype=torch.float32, generator=gen) * 0.5).to(torch.bfloat16)
+    fp8 = args.dtype == "fp8"
     pools, qs, kns, vns, outs = [], [], [], [], []
     for l in range(L):
-        kp = torch.empty(w.n_pages, H, P, D, device=dev, dtype=torch.bfloat16)
-        vp = torch.empty_like(kp)
-        for t in (kp, vp):                             # fill page by page-block to bound the fp32 temporary
-            for a in range(0, w.n_pages, 64):
-                t[a:a + 64] = rnd(min(64, w.n_pages - a), H, P, D)
-        pools.append(binding.Pool(kp, vp, w.n_pages, H, D, P, "bf16"))
+        if fp8:
+            # e4m3 codes of the same N(0, 0.25) values under one scale per block (5 sigma / 448); torch's cast only builds
+            # the synthetic cache contents here - every chunk the bench appends is quantised by slack_kv_append itself
+            sc = 2.5 / 448.0
+            kp = torch.empty(w.n_pages, H, P, D, device=dev, dtype=torch.uint8)
+            vp = torch.empty_like(kp)
+            for t in (kp, vp):
+                for a in range(0, w.n_pages, 64):
+                    t[a:a + 64] = (rnd(min(64, w.n_pages - a), H, P, D).float() / sc).to(torch.float8_e4m3fn).view(torch.uint8)
+            ks = torch.full((w.n_pages, H, P // 128), sc, device=dev, dtype=torch.float32)
+            pools.append(binding.Pool(kp, vp, w.n_pages, H, D, P, "fp8", k_scale=ks, v_scale=ks.clone()))
+        else:
+            kp = torch.empty(w.n_pages, H, P, D, device=dev, dtype=torch.bfloat16)
+            vp = torch.empty_like(kp)
+            for t in (kp, vp):                             # fill page by page-block to bound the fp32 temporary
+                for a in range(0, w.n_pages, 64):
+                    t[a:a + 64] = rnd(min(64, w.n_pages - a), H, P, D)
+            pools.append(binding.Pool(kp, vp, w.n_pages, H, D, P, "bf16"))
         qs.append(rnd(tq, H, D)); kns.append(rnd(tq, H, D)); vns.append(rnd(tq, H, D))
         outs.append(torch.empty(tq, H, D, device=dev, dtype=torch.bfloat16))
     main = torch.cuda.current_stream()
@@ -466,12 +481,17 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
     which = "MEASURED_PEAKS.json bf16_tflops (burst: SURVEY.md A11 headline denominator)" if "bf16_tflops" in peaks else \
         "fallback: B200_PROFILING.md 1.59 PFLOP/s burst (MEASURED_PEAKS.json absent)"
     sustained = float(peaks["bf16_tflops_sustained"]) if "bf16_tflops_sustained" in peaks else None
+    if fp8:   # a contraction takes the peak of its own dtype: the measured bf16 figure x the nominal fp8 : bf16 ratio of 2
+        burst, sustained = 2.0 * burst, (2.0 * sustained if sustained else None)
+        which += " x 2 (nominal fp8 : bf16 ratio, B200_PROFILING.md)"
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     kernel_ms = k_ms / max(k_n, 1)
     achieved = flops_layer / (kernel_ms * 1e-3) / 1e12 if k_n else None
     # minimal HBM bytes of one launch: Q read, Out written, every visible K and V read once per (stream, head)
     bytes_layer = metrics.attention_min_bytes(w.streams, H, D, 2)
+    if fp8:   # K and V are one byte per element; Q and Out stay bf16
+        bytes_layer = float(sum((2 * s.q_len * 2 + 2 * lk * 1) * H * D for s, lk in zip(w.streams, metrics.visible_keys(w.streams))))
     intensity = flops_layer / bytes_layer
     traffic, traffic_src = NCU_TRAFFIC_BYTES.get(name if (layer_masks is None and (name != "cfg5" or args.kv_chunks == 7)) else "", (None, None))
     stats = lambda xs: {"ms_avg": float(np.mean(xs)), "ms_median": float(np.median(xs)), "ms_min": float(np.min(xs)),
@@ -493,7 +513,7 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
                     "frac_of_sustained": (achieved / sustained) if achieved and sustained else None,
                     "frac_of_nominal_2250": (achieved / 2250.0) if achieved else None,
                     "kernel_share_of_step": (k_ms / ms_prof) if k_n else None}
-    app_bytes = metrics.append_bytes(w.streams, H, D, 2)
+    app_bytes = metrics.append_bytes(w.streams, H, D, 2) * (0.75 if fp8 else 1.0)   # fp8: bf16 read, 1-byte codes written
     append = stats(a_list)
     if append:
         append.update(kernel="kv_append_kernel", bytes_per_launch=app_bytes, GB_per_s=app_bytes / (append["ms_avg"] * 1e-3) / 1e9,
@@ -506,7 +526,23 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
 
     # ---- CPU baseline: the oracle on layer 0 of this very run (also a live parity spot check) ----------------------
     cpu, parity = None, None
-    if want_cpu and rank == 0:
+    if want_cpu and rank == 0 and fp8:
+        # the FP8 oracle (oracle/fp8_attention.py) on a row sample of layer 0: dequantised operands, exact P
+        import oracle
+        Fo = oracle.fp8_attention
+        img = [t.cpu().numpy() for t in (pools[0].k_pool, pools[0].v_pool, pools[0].k_scale, pools[0].v_scale)]
+        q0 = binding.to_numpy(qs[0], "bf16")
+        rows = sample_rows(w.streams, 256)
+        t0 = time.perf_counter()
+        o_want, _ = Fo.chunk_attention_fp8(img[0], img[1], img[2], img[3], w.streams, q0, w.scale, "bf16", rows=rows)
+        dt = time.perf_counter() - t0
+        fl = sample_flops(w.streams, rows, H, D)
+        ma, rf = oracle.error_metrics(outs[0].float().cpu().numpy().astype(np.float64), o_want)
+        parity = {"rows": int(sum(len(r) for r in rows)), "max_abs": ma, "rel_fro": rf, "pass": bool(ma <= 2e-2 and rf <= 4e-2),
+                  "against": "oracle.fp8_attention.chunk_attention_fp8 (dequantised Q, K, V; exact P); gate rel-Fro 4e-2"}
+        cpu = {"value": fl / dt / 1e12, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "seconds": dt,
+               "sample": f"{parity['rows']} seeded query rows x {H} heads x all visible keys of layer 0 (fp64 numpy, incl. dequantising the pool)"}
+    elif want_cpu and rank == 0:
         kp0 = binding.to_numpy(pools[0].k_pool, "bf16")
         vp0 = binding.to_numpy(pools[0].v_pool, "bf16")
         q0 = binding.to_numpy(qs[0], "bf16")
@@ -560,7 +596,7 @@ def run_ours(args):
 
     # ---- supplementary blocks (N = 1 only): the other things `metric` / `north_star` name, a few steps each -----------
     others = {}
-    if world == 1 and not args.no_others and args.sparsity == 0 and args.workload == "cfg5":
+    if world == 1 and not args.no_others and args.sparsity == 0 and args.workload == "cfg5" and args.dtype == "bf16":
         for name, why in (("cfg4", "configs[3] mixed streams: chunks/s"), ("cfg3", "configs[2]: the 460 MB append"),
                           ("cfg5b", "decode-like short chunks: HBM GB/s")):
             gc.collect()
@@ -586,9 +622,10 @@ def run_ours(args):
         return
 
     line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16" if args.dtype == "bf16" else "fp8_e4m3 (K/V pool codes, Q and P quantised online; fp32 accumulation; bf16 in/out)",
             "data": "synthetic",
-            "config": {"workload": workload_label(args, w), "layers_per_step": r["layers"], "streams": len(w.streams),
+            "config": {"workload": workload_label(args, w) + ("" if args.dtype == "bf16" else " [FP8 pool variant, NEXT-3]"), "layers_per_step": r["layers"], "streams": len(w.streams),
                        "l2": "inputs larger than L2: every layer has its own pools (no flush needed)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "plan": r["plan_info"],
                        "flops_per_step": r["job_flops_step"], "chunk_layers_per_s": r["chunk_layers_per_s"],

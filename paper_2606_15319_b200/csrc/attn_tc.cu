@@ -231,7 +231,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         for (int j0 = 0; j0 < Ts; j0 += 32) { // 32 steps at a time: each lane looks up the pool row of one step's tile
           const int my_jj = j0 + lane;
           int my_row = 0;
-          float my_sk = 1.f, my_sv = 1.f;
+          [[maybe_unused]] float my_sk = 1.f, my_sv = 1.f;
           if (my_jj < Ts) {
             const int my_tile = v.tile_of(kSparse ? (int)__ldg(steps + my_jj) : my_jj);
             const int my_page = __ldg(p.page_tables + pt_off + ((my_tile * kTileN) >> p.page_log2));
@@ -245,7 +245,11 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           const int cnt = min(32, Ts - j0);
           for (int j = 0; j < cnt; ++j) {
             const int row = __shfl_sync(0xffffffffu, my_row, j);
-            [[maybe_unused]] const float t_sk = __shfl_sync(0xffffffffu, my_sk, j), t_sv = __shfl_sync(0xffffffffu, my_sv, j);
+            [[maybe_unused]] float t_sk = 1.f, t_sv = 1.f;
+            if constexpr (kFp8) {
+              t_sk = __shfl_sync(0xffffffffu, my_sk, j);
+              t_sv = __shfl_sync(0xffffffffu, my_sv, j);
+            }
 #pragma unroll
             for (int kv = 0; kv < 2; ++kv) {
               const uint32_t stage = ring % kStages;

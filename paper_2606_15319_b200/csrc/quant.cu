@@ -4,9 +4,9 @@
 // divisions IEEE fp32 (__fdiv_rn), so that codes and scales are bit-exact against the oracle.
 //
 //   kv_append_fp8_kernel  A1 for FP8 pools: one CTA per (key block of 128 slots, head, stream x {K, V}); a block whose
-//                         first held token this append writes gets its scale from the tokens written (pass 1: amax),
-//                         any other block keeps the stored scale; pass 2 writes the codes (one warp per token row).
-//                         HBM-bound: reads 2 * Lq * H * D * 2 B (bf16; the second pass hits L2), writes half of that.
+//                         first held token this append writes gets its scale from the tokens written, any other
+//                         block keeps the stored scale.  The block's rows (<= 128 x 256 B) stay in registers between
+//                         the amax and the conversion: HBM-bound, 2 * Lq * H * D * 2 B read once, half of that written.
 //   q_quant_kernel        Q of an attention call -> codes [sum Lq][H][128] + scales [H][sum Lq] in the workspace;
 //                         one warp per (row, head).
 #include <cuda_bf16.h>
@@ -69,18 +69,26 @@ kv_append_fp8_kernel(const uint2 *__restrict__ k_new, const uint2 *__restrict__ 
   const int tok0 = p_first - s.app_pos0; // chunk-local index of the first token written here
   // source row of (token, head): 128 bf16 = 32 lanes x 8 bytes
   auto src_of = [&](int t) { return src + ((size_t)(s.q_row0 + tok0 + t) * n_heads + h) * 32 + lane; };
-  __shared__ float red[kQuantThreads / 32];
+  // every warp keeps its (at most 16) token rows in registers: the source is read from HBM once
+  constexpr int kWarps = kQuantThreads / 32, kRowsPerWarp = 128 / kWarps;
+  uint2 rows[kRowsPerWarp];
+  float am = 0.f;
+#pragma unroll
+  for (int r = 0; r < kRowsPerWarp; ++r) {
+    const int t = warp + r * kWarps;
+    rows[r] = t < n_tok ? __ldcs(src_of(t)) : make_uint2(0u, 0u);
+    am = fmaxf(am, amax4(rows[r]));
+  }
+  __shared__ float red[kWarps];
   __shared__ float scale_sh;
   if (!has_old) {
-    float am = 0.f;
-    for (int t = warp; t < n_tok; t += kQuantThreads / 32) am = fmaxf(am, amax4(__ldg(src_of(t))));
     am = warp_max(am);
     if (lane == 0) red[warp] = am;
     __syncthreads();
     if (threadIdx.x == 0) {
       float a = red[0];
 #pragma unroll
-      for (int w = 1; w < kQuantThreads / 32; ++w) a = fmaxf(a, red[w]);
+      for (int w = 1; w < kWarps; ++w) a = fmaxf(a, red[w]);
       const float sc = a > 0.f ? __fdiv_rn(a, kE4m3Max) : 1.0f;
       scale_sh = sc;
       *scale_ptr = sc;
@@ -92,9 +100,13 @@ kv_append_fp8_kernel(const uint2 *__restrict__ k_new, const uint2 *__restrict__ 
   const float sc = scale_sh;
   // destination row of position p, head h: 128 codes = 32 lanes x 4 bytes
   const int page_mask = (1 << page_log2) - 1;
-  for (int t = warp; t < n_tok; t += kQuantThreads / 32) {
-    const int slot = (p_first + t) & page_mask;
-    pool[((((size_t)page * n_heads + h) << page_log2) + slot) * 32 + lane] = quant4(__ldg(src_of(t)), sc);
+#pragma unroll
+  for (int r = 0; r < kRowsPerWarp; ++r) {
+    const int t = warp + r * kWarps;
+    if (t < n_tok) {
+      const int slot = (p_first + t) & page_mask;
+      pool[((((size_t)page * n_heads + h) << page_log2) + slot) * 32 + lane] = quant4(rows[r], sc);
+    }
   }
 }
 

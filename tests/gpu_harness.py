@@ -14,6 +14,9 @@ import oracle
 from paper_2606_15319_b200 import binding
 from helpers import oracle_pools, prior_batches
 
+# kernel kind the tensor-core cases report: 0, or 2 when SLACK_TEST_CTA_PAIRS=2 reruns the suites on CTA pairs
+TC_KIND = 2 if os.environ.get("SLACK_TEST_CTA_PAIRS", "0") == "2" else 0
+
 SENTINEL_BF16 = 0x7FC1   # a NaN bit pattern: any leak of an unowned / masked slot into the output shows up as NaN
 SENTINEL_F32 = np.float32(np.nan)
 

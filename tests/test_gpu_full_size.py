@@ -63,7 +63,7 @@ def full_case(ctx, w, check_append=True, full_output=True, **opts):
     if full_output:
         assert not np.isnan(want).any()
     res = G.check_attention(w, out, lse, want, want_lse)
-    assert plan.kernel_kind == 0
+    assert plan.kernel_kind == G.TC_KIND
     return res, plan
 
 

@@ -78,7 +78,7 @@ def test_cfg1_fp32_simt(ctx):
 @pytest.mark.parametrize("splits", [0, 1, 2, 3])
 def test_small_ragged_tensor_core(ctx, page_size, splits):
     res, *_ = run_case(ctx, W.small_ragged(page_size=page_size), force_splits=splits)
-    assert res["kind"] == 0
+    assert res["kind"] == G.TC_KIND
 
 
 # ------------------------------------------------------------------------------------------------ sink + local
@@ -88,7 +88,7 @@ def test_sink_plus_local_window_tensor_core(ctx, page_size, splits):
     """Visible keys = [0, sink) U [max(sink, lo), n): the sink tiles are visited before the window tiles of the first
     piece of every row; sink ends mid-tile, shares a tile with the window start, or is absorbed by the window."""
     res, *_ = run_case(ctx, W.sink_ragged(page_size=page_size), force_splits=splits)
-    assert res["kind"] == 0
+    assert res["kind"] == G.TC_KIND
 
 
 @pytest.mark.parametrize("page_size", [128, 256])
@@ -101,7 +101,7 @@ def test_bounded_sink_cache_with_hole(ctx, page_size, splits):
     G.gpu_append_all(ctx, w, pool)
     assert G.pools_equal_oracle(w, pool)
     res, *_ = run_case(ctx, w, force_splits=splits)
-    assert res["kind"] == 0
+    assert res["kind"] == G.TC_KIND
 
 
 def test_bounded_sink_cache_with_hole_simt(ctx):
@@ -237,7 +237,7 @@ def test_unusual_shapes_sampled_rows(ctx, n_heads, page_size, lq, lc, window, ba
     rows = [np.unique(np.concatenate([[0, 127, 128, lq - 1], np.random.default_rng(5).integers(0, lq, size=24)]))]
     for splits in (0, 1):
         res, out, *_ = run_case(ctx, w, rows=rows, force_splits=splits)
-        assert res["kind"] == 0
+        assert res["kind"] == G.TC_KIND
 
 
 # ------------------------------------------------------------------------------------------------ plan / staging lifetime
@@ -256,7 +256,7 @@ def test_plans_created_and_destroyed_while_kernels_are_in_flight(ctx):
     torch.cuda.synchronize()
     for it in range(300):
         st = streams[it & 1]
-        plan = ctx.slack_plan(pool, w.streams, force_splits=2)
+        plan = ctx.slack_plan(pool, w.streams, force_splits=2, cta_pairs=plan0.kernel_kind)   # 0 (automatic) or 2
         ctx.slack_chunk_attention(plan, pool, q, outs[it & 1], w.scale, workspace=wss[it & 1], stream=st)
         plan.close()
     torch.cuda.synchronize()

@@ -133,7 +133,7 @@ def test_layer_major_events_and_attention_after_rehoming(ctx):
         out, lse, plan, _ = G.gpu_attention(ctx, w, dsts[l])
         want, want_lse = G.oracle_attention(ws[l])
         G.check_attention(ws[l], out, lse, want, want_lse)
-        assert plan.kernel_kind == 0
+        assert plan.kernel_kind == G.TC_KIND
 
 
 def test_transfer_argument_errors(ctx):
