@@ -502,7 +502,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         // logit -> exponent: z = s * cz + az.  bf16: cz = scale log2e, az = 0 and m is kept in units of s (z = s cz).
         // FP8: cz = scale log2e sq sk_t, az = log2 sv_t (the V scale rides inside P), m is kept in units of z, and P is
         // scaled by 2^7 so that its e4m3 codes use the range up to 128 (x 2 before a lazy rescale) of the format's 448.
-        float cz = sl2, az = 0.f, l_fix = 1.f;
+        [[maybe_unused]] float cz = sl2, az = 0.f, l_fix = 1.f;
         if constexpr (kFp8) {
           const float t_sk = ld_shared_f32(sScale + ((r0 + 2u * (uint32_t)j) % kScaleRing) * 4u);
           const float t_sv = ld_shared_f32(sScale + ((r0 + 2u * (uint32_t)j + 1u) % kScaleRing) * 4u);
@@ -510,14 +510,20 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           az = log2f(t_sv);
           l_fix = 0.0078125f / t_sv; // this tile's P sums, taken in units of 128 sv_t, back to plain probabilities
         }
-        auto to_m = [&](float mx_s) { return kFp8 ? fmaf(mx_s, cz, az) : mx_s; };       // row max of s -> units of m
-        auto neg_m = [&]() { return kFp8 ? (az - m + 7.0f) : (-m * sl2); };               // addend of the exponent
+        auto to_m = [&](float mx_s) { // row max of s -> units of m
+          if constexpr (kFp8) return fmaf(mx_s, cz, az);
+          else return mx_s;
+        };
+        auto neg_m = [&]() { // addend of the exponent
+          if constexpr (kFp8) return az - m + 7.0f;
+          else return -m * sl2;
+        };
         constexpr float kThr = kFp8 ? kRescaleThreshold8 : kRescaleThreshold;
         if (j == 0) m = to_m(row_max());
         SLACK_TRACE(i, j, 3);
         // P = 2^(s*cz + addend) on packed pairs: FFMA2 for the argument, then either 2 MUFU.EX2 or (kEmuOf8 pairs out
         // of every 8) the FMA-pipe polynomial; FADD2 row sums; one F2FP per pair (FP8: per four).
-        const uint64_t sl2_2 = pack2(cz, cz);
+        const uint64_t sl2_2 = kFp8 ? pack2(cz, cz) : pack2(sl2, sl2);
         uint64_t negm_2 = pack2(neg_m(), neg_m());
         uint64_t la0 = pack2(0.f, 0.f), la1 = la0;
         auto exp_chunk = [&](int c) { // 32 columns -> 16 packed bf16x2 (FP8: 8 packed e4m3x4) columns of P
@@ -556,13 +562,16 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         auto flush_sums = [&]() {
           float a0, a1;
           unpack2(fadd2(la0, la1), a0, a1);
-          l = fmaf(a0 + a1, l_fix, l);
+          if constexpr (kFp8) l = fmaf(a0 + a1, l_fix, l);
+          else l += a0 + a1;
         };
         {
           const float mx = to_m(row_max()); // independent of the two chunks below: the scheduler interleaves them
           exp_chunk(0);
           exp_chunk(1);
-          const float grow = kFp8 ? (mx - m) : (mx - m) * sl2;
+          float grow;
+          if constexpr (kFp8) grow = mx - m;
+          else grow = (mx - m) * sl2;
           const bool need = grow > kThr; // never on the first tile (m == mx)
           if (__any_sync(0xffffffffu, need)) {
             // PV of the previous key tile has completed (its commit precedes S_FULL in the in-order tensor pipe)

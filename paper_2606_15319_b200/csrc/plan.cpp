@@ -36,7 +36,9 @@ void set_sink(DevItem &it, const StreamGeom &g, const DevStream &s, bool first_p
 }
 
 constexpr double kTileCost = 2.0;      // one 128-key tile against a 256-row item (two MMA tile pairs)
-constexpr double kItemOverhead = 9.0;  // pipeline fill/drain + epilogue: measured ~15k cycles = 4.4 steps of 3400 (per-CTA span fit)
+constexpr double kItemOverhead = 7.75; // pipeline fill/drain + epilogue: 12.6k cycles = 3.9 steps of 3250 (least-squares fit of per-CTA
+                                       // spans on BASELINE configs 2, 4, 5: cycles = 3250 x two-tile steps + 2755 x one-tile steps + 12.6k x items)
+constexpr double kTileCost1 = 1.70; // one 128-key tile against a single query tile: 2755 vs 3250 cycles (same fit; the chain bounds it)
 constexpr double kPartialCost = 3.0;   // extra epilogue traffic + combine work per partial slot
 
 struct Candidate {
@@ -51,7 +53,7 @@ int32_t ceil_div(int64_t a, int64_t b) { return (int32_t)((a + b - 1) / b); }
 
 // parts[s] = number of key chunks for stream s
 void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int32_t> &parts,
-                    const std::vector<DevStream> &ds, int32_t n_heads, int32_t n_cta, Candidate &c) {
+                    const std::vector<DevStream> &ds, int32_t n_heads, int32_t n_cta, bool pairs, Candidate &c) {
   c = Candidate();
   for (size_t oi = 0; oi < order.size(); ++oi) {
     const StreamGeom &g = order[oi];
@@ -100,7 +102,8 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
   c.item_cta.resize(c.items.size());
   double total = 0;
   for (size_t i = 0; i < c.items.size(); ++i) {
-    const double cost = kTileCost * (c.items[i].kv_tile_end - c.items[i].kv_tile_begin + c.items[i].sink_tiles) + kItemOverhead;
+    const double tc = (pairs || c.items[i].q_rows > kTileM) ? kTileCost : kTileCost1;
+    const double cost = tc * (c.items[i].kv_tile_end - c.items[i].kv_tile_begin + c.items[i].sink_tiles) + kItemOverhead;
     Slot s = heap.top();
     heap.pop();
     c.item_cta[i] = s.second;
@@ -123,7 +126,6 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
 // well but de-synchronises the sweeps: measured 17 % slower on BASELINE config 5, its K/V working set leaving L2.)
 constexpr int32_t kMinPiece = 4;
 constexpr bool kAutoPairs = false; // automatic plans use CTA pairs where they pay (see build_plan)
-constexpr double kTileCost1 = 1.55; // one 128-key tile against a single query tile: measured 2620 vs 3400 cycles (the chain bounds it)
 
 struct Row {
   int32_t oi, head, qb, q_rows, tile0, tiles, sink_tiles;
@@ -237,10 +239,28 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
       }
     }
   }
-  while (ti < tail.size()) { // what rounding and the minimum piece length left over: to the least loaded queue
-    const int32_t cta = (int32_t)(std::min_element(load.begin(), load.end()) - load.begin());
-    emit(tail[ti], tb, rem, cta);
-    close_row();
+  // What rounding and the minimum piece length left over: dealt out in pieces to the least loaded queues, each topped up to
+  // the level all queues would reach if the leftovers were spread evenly (never a whole row on one queue unless it fits).
+  if (ti < tail.size()) {
+    double left = tail[ti].tc * rem + kItemOverhead;
+    for (size_t t2 = ti + 1; t2 < tail.size(); ++t2) left += tail[t2].tc * (tail[t2].tiles + tail[t2].sink_tiles) + kItemOverhead;
+    double have = 0;
+    for (double v : load) have += v;
+    const double level = (have + left) / n_cta + 2 * kItemOverhead;
+    while (ti < tail.size()) {
+      const int32_t cta = (int32_t)(std::min_element(load.begin(), load.end()) - load.begin());
+      const Row &r = tail[ti];
+      int32_t take = (int32_t)std::floor((level - load[cta] - kItemOverhead) / r.tc) - (tb == r.tile0 ? r.sink_tiles : 0);
+      take = std::max(take, kMinPiece);
+      if (take >= rem || rem - take < kMinPiece) {
+        emit(r, tb, rem, cta);
+        close_row();
+      } else {
+        emit(r, tb, take, cta);
+        tb += take;
+        rem -= take;
+      }
+    }
   }
   c.ideal = total / n_cta;
   for (double v : load) c.makespan = std::max(c.makespan, v);
@@ -420,7 +440,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
       }
     }
     Candidate c;
-    make_candidate(order, parts, out.streams, shape.n_heads, n_queues, c);
+    make_candidate(order, parts, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, c);
     if (!have || c.objective < best.objective - 1e-9) {
       best = std::move(c);
       have = true;
