@@ -137,6 +137,8 @@ typedef struct {
   int32_t sink_pos_hi;   /* base + sink_len when the item visits sink tiles, else base                            */
   int32_t partial_slot;  /* -1: writes `out` directly; >= 0: writes workspace slot (split-KV), combined afterwards */
   int32_t cta;           /* queue that holds this item: CTA 0..sm_count-1, or CTA pair 0..sm_count/2-1 (pair plans) */
+  int32_t dual;          /* 1: this item and the NEXT one of the same queue (both <= 128 rows, same number of key tiles)
+                            are walked together by one CTA, one per query-tile slot (decode-like chunks, 72-row tails) */
 } slack_work_item;
 
 /* ---- context ------------------------------------------------------------------------------------------------ */

@@ -45,7 +45,7 @@ class CPlanOpts(C.Structure):
 
 class CWorkItem(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("stream", "head", "q_row0", "q_rows", "kv_tile_begin", "kv_tile_end",
-                                         "pos_lo", "pos_hi", "sink_tiles", "sink_pos_hi", "partial_slot", "cta")]
+                                         "pos_lo", "pos_hi", "sink_tiles", "sink_pos_hi", "partial_slot", "cta", "dual")]
 
 
 # every symbol include/slack.h declares: name -> (restype, argtypes)

@@ -539,6 +539,7 @@ int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, i
     w.sink_pos_hi = d.sink_hi;
     w.partial_slot = d.partial_slot;
     w.cta = hp.item_cta[i];
+    w.dual = d.dual;
   }
   return n;
 }
@@ -790,6 +791,7 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
   while ((1 << pl2) < hp.page_size) ++pl2;
   p.page_log2 = pl2;
   p.total_q = hp.total_q;
+  p.has_dual = hp.has_dual ? 1 : 0;
   p.scale = scale;
   if (fp8) {
     p.k_scale = pool->k_scale;

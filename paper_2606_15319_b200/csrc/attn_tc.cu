@@ -15,6 +15,12 @@
 // other tile's P V and next Q K^T.  TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_i is
 // written over the first 64 columns of S_i (two bf16 per 32-bit column).
 //
+// Dual items (DevItem::dual; dense bf16 instantiation only): two single-tile items (<= 128 query rows each: decode-like
+// chunks, the 72-row tails of long chunks) of the same number of key steps share the CTA, one per query-tile slot, each
+// with its OWN K/V tiles (ring entries K_a V_a K_b V_b per step): the idle slot of a single-tile item is filled, the key
+// step costs what a two-tile step costs (3250 cycles) instead of 2 x 2755, and an HBM-bound batch keeps twice the
+// bytes in flight per SM.  The other instantiations walk the two items one after the other.
+//
 // Block-sparse variant (kSparse, PAPER.md P:88 knob (2) "skips nonselected attention blocks with
 // sparse masks"): an item visits only the key-tile steps listed for it by sparse_steps.cu (the device block mask changes
 // per layer / denoising step, the host plan does not); every role walks that list instead of 0..T-1, an item with an
@@ -134,10 +140,13 @@ __device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
       p.dbg_t[((role) * 64 + (step)) * 8 + (slot)] = (uint32_t)clock64();                                  \
   }
 
-template <bool kTrace, bool kSparse, bool kFp8>
+template <bool kTrace, bool kSparse, bool kFp8, bool kDual = false>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                const __grid_constant__ CUtensorMap tm_v) {
+  // dual items (DevItem::dual) are served by a dense bf16 instantiation of their own, launched for plans that hold any:
+  // carrying the extra paths costs the issuer warp registers (spills on its critical path: +4.6 % cycles per key step)
+  constexpr bool kDualOk = kDual && !kSparse && !kFp8;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base + kOffQ;
@@ -213,25 +222,38 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         if (Ts == 0) continue;
         const uint16_t *steps = kSparse ? p.steps + uni(it.step_off) : nullptr;
         const int head = uni(it.head), q_row0 = uni(it.q_row0), pt_off = uni(it.pt_off);
+        // dual item: the queue's next item rides in query-tile slot 1 with its own head / rows / page table / key tiles
+        const bool dual = kDualOk && uni(it.dual) != 0;
+        const DevItem itb = dual ? p.items[k + 1] : it;
+        const ItemView vb = uniform_view_of(itb);
+        const int head_b = uni(itb.head), q_row0_b = uni(itb.q_row0), pt_off_b = uni(itb.pt_off);
+        const int nq = dual ? 2 : v.nq;
         mbar_wait(bar(BAR_Q_EMPTY), (uint32_t)((n_item & 1) ^ 1), 100, dbg);
         ++n_item;
         if (elect_one()) {
           if constexpr (kFp8) { // one [128 rows][128 codes] box per query tile
-            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes8);
-            for (int i = 0; i < v.nq; ++i) tma_load_2d(sQ + i * kTileBytes, &tm_q, bar(BAR_Q_FULL), head * 128, q_row0 + i * kTileM);
+            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytes8);
+            for (int i = 0; i < nq; ++i) tma_load_2d(sQ + i * kTileBytes, &tm_q, bar(BAR_Q_FULL), head * 128, q_row0 + i * kTileM);
           } else {
-            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)v.nq * kTileBytes);
-            for (int i = 0; i < v.nq; ++i)
+            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytes);
+            for (int i = 0; i < nq; ++i) {
+              const int h_i = (dual && i == 1) ? head_b : head;
+              const int r_i = (dual && i == 1) ? q_row0_b : q_row0 + i * kTileM;
               for (int c = 0; c < 2; ++c)
-                tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), head * 128 + c * 64,
-                            q_row0 + i * kTileM);
+                tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), h_i * 128 + c * 64, r_i);
+            }
           }
         }
         __syncwarp();
         for (int j0 = 0; j0 < Ts; j0 += 32) { // 32 steps at a time: each lane looks up the pool row of one step's tile
           const int my_jj = j0 + lane;
-          int my_row = 0;
+          int my_row = 0, my_row_b = 0;
           [[maybe_unused]] float my_sk = 1.f, my_sv = 1.f;
+          if (dual && my_jj < Ts) {
+            const int tile_b = vb.tile_of(my_jj);
+            const int page_b = __ldg(p.page_tables + pt_off_b + ((tile_b * kTileN) >> p.page_log2));
+            my_row_b = (page_b * H + head_b) * P + ((tile_b * kTileN) & (P - 1));
+          }
           if (my_jj < Ts) {
             const int my_tile = v.tile_of(kSparse ? (int)__ldg(steps + my_jj) : my_jj);
             const int my_page = __ldg(p.page_tables + pt_off + ((my_tile * kTileN) >> p.page_log2));
@@ -244,12 +266,15 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           }
           const int cnt = min(32, Ts - j0);
           for (int j = 0; j < cnt; ++j) {
-            const int row = __shfl_sync(0xffffffffu, my_row, j);
+            const int row_a = __shfl_sync(0xffffffffu, my_row, j);
+            const int row_b = dual ? __shfl_sync(0xffffffffu, my_row_b, j) : 0;
             [[maybe_unused]] float t_sk = 1.f, t_sv = 1.f;
             if constexpr (kFp8) {
               t_sk = __shfl_sync(0xffffffffu, my_sk, j);
               t_sv = __shfl_sync(0xffffffffu, my_sv, j);
             }
+            for (int t = 0; t < (dual ? 2 : 1); ++t) { // dual: K_a V_a K_b V_b
+            const int row = t == 0 ? row_a : row_b;
 #pragma unroll
             for (int kv = 0; kv < 2; ++kv) {
               const uint32_t stage = ring % kStages;
@@ -270,8 +295,10 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
               __syncwarp();
               ++ring;
             }
+            }
           }
         }
+        if (dual) ++k; // the companion has been served
       }
     } else if (warp == 1) {
       // ============================== MMA issuer ==============================
@@ -330,6 +357,86 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         const uint32_t r0 = ring;
         mbar_wait(bar(BAR_Q_FULL), (uint32_t)(n_item & 1), 200, dbg);
         ++n_item;
+        // masked key rows of a V tile must be zero: P is 0 there, but 0 * NaN/Inf garbage would poison O
+        auto zero_masked_v = [&](const ItemView &vv, int jd, uint32_t stage) {
+          const int tile = vv.tile_of(jd);
+          const int c_lo = max(0, vv.lo_of(jd) - tile * kTileN);
+          const int c_hi = min(kTileN, vv.hi_of(jd) - tile * kTileN);
+          if (c_lo > 0 || c_hi < kTileN) {
+            const int n_zero = c_lo + (kTileN - c_hi);
+            const uint32_t base = sKV + stage * kTileBytes;
+            for (int idx = lane; idx < n_zero * 16; idx += 32) {
+              int r = idx >> 4;
+              r = r < c_lo ? r : c_hi + (r - c_lo);
+              const int w = idx & 15;
+              const uint32_t addr = base + (uint32_t)(w >> 3) * kHalfBytes + (uint32_t)r * 128u + (uint32_t)(w & 7) * 16u;
+              asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+          }
+        };
+        if (kDualOk && uni(it.dual) != 0) {
+          // ---- dual item: tile slot i walks its own item (k + i) over its own ring entries K_i(j) = r0 + 4j + 2i, V_i(j) = K_i(j) + 1
+          const DevItem itb = p.items[k + 1];
+          const ItemView vb = uniform_view_of(itb);
+          auto entry = [&](int i, int j, int kv, uint32_t &stage, uint32_t &ph) {
+            const uint32_t r = r0 + 4u * (uint32_t)j + 2u * (uint32_t)i + (uint32_t)kv;
+            stage = r % kStages;
+            ph = (r / kStages) & 1u;
+          };
+          for (int i = 0; i < 2; ++i) {
+            uint32_t stage, ph;
+            entry(i, 0, 0, stage, ph);
+            mbar_wait(bar(BAR_KV_FULL + stage), ph, 210 + stage, dbg);
+            tc_fence_after();
+            if (elect_one()) {
+              issue_qk(i, stage);
+              mma_commit(bar(BAR_S_FULL + i));
+              mma_commit(bar(BAR_KV_EMPTY + stage));
+              if (Ts == 1 && i == 1) mma_commit(bar(BAR_Q_EMPTY));
+            }
+            __syncwarp();
+          }
+          for (int j = 0; j < Ts; ++j) {
+            const bool has_next = (j + 1) < Ts;
+            for (int i = 0; i < 2; ++i) {
+              uint32_t stage_v, ph_v, stage_k = 0, ph_k = 0;
+              entry(i, j, 1, stage_v, ph_v);
+              mbar_wait(bar(BAR_KV_FULL + stage_v), ph_v, 220 + stage_v, dbg);
+              zero_masked_v(i == 0 ? v : vb, j, stage_v);
+              mbar_wait(bar(BAR_P_LO + i), cnt[i] & 1u, 260 + i, dbg);
+              if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
+              tc_fence_after();
+              if (elect_one()) issue_pv(i, stage_v, 0, j > 0);
+              __syncwarp();
+              mbar_wait(bar(BAR_P_READY + i), cnt[i] & 1u, 230 + i, dbg);
+              if (has_next) {
+                entry(i, j + 1, 0, stage_k, ph_k);
+                mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
+              }
+              tc_fence_after();
+              if (elect_one()) {
+                issue_pv(i, stage_v, 1, true);
+                mma_commit(bar(BAR_KV_EMPTY + stage_v));
+                if (has_next) {
+                  issue_qk(i, stage_k);
+                  mma_commit(bar(BAR_S_FULL + i));
+                  mma_commit(bar(BAR_KV_EMPTY + stage_k));
+                  if (i == 1 && j + 2 == Ts) mma_commit(bar(BAR_Q_EMPTY));
+                } else {
+                  mma_commit(bar(BAR_O_FINAL + i));
+                }
+              }
+              __syncwarp();
+              cnt[i]++;
+              if (!has_next) itn[i]++;
+            }
+          }
+          ring = r0 + 4u * (uint32_t)Ts;
+          ++k; // the companion has been served
+          continue;
+        }
         {
           const uint32_t stage = r0 % kStages, ph = (r0 / kStages) & 1u;
           mbar_wait(bar(BAR_KV_FULL + stage), ph, 210 + stage, dbg);
@@ -422,16 +529,21 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
     uint32_t cnt = 0, itn = 0;
     [[maybe_unused]] uint32_t ring = 0; // FP8: ring entry of the item's first K tile (the producer's count; scale slots)
     bool first_item = true;
-    for (int k = item_begin; k < item_end; ++k) {
-      const DevItem it = p.items[k];
+    int adv = 1;
+    for (int k = item_begin; k < item_end; k += adv) {
+      // dual item: tile slot 1 serves the queue's NEXT item (its own rows 0.., head, mask columns, output rows)
+      const bool dual = kDualOk && p.items[k].dual != 0;
+      adv = dual ? 2 : 1;
+      const DevItem it = p.items[k + ((dual && i == 1) ? 1 : 0)];
       const ItemView v = view_of(it);
+      const int row_base = dual ? 0 : i * kTileM; // this tile's first row inside ITS item
       [[maybe_unused]] const uint32_t r0 = ring;
       if constexpr (kFp8) ring += 2u * (uint32_t)v.T; // every role counts the item's tiles, also the one that skips it
-      if (i >= v.nq) continue;
+      if (!dual && i >= v.nq) continue;
       const int Ts = kSparse ? p.item_steps[k] : v.T;
       const uint16_t *steps = kSparse ? p.steps + it.step_off : nullptr;
       if (Ts == 0) { // block-sparse: no selected key tile in this item: out = 0, lse = -inf; no barrier is touched
-        const int local_row = i * kTileM + row;
+        const int local_row = row_base + row;
         if (local_row < it.q_rows) {
           if (it.partial_slot < 0) {
             uint4 *dst = reinterpret_cast<uint4 *>(reinterpret_cast<__nv_bfloat16 *>(p.out) +
@@ -616,7 +728,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       mbar_wait(bar(BAR_O_FINAL + i), itn & 1u, 310 + i, dbg);
       tc_fence_after();
       const float inv_l = kFp8 ? 0.0078125f / l : 1.0f / l; // FP8: O was accumulated from P = 128 * probabilities
-      const int local_row = i * kTileM + row;
+      const int local_row = row_base + row;
       const bool valid = local_row < it.q_rows;
       const float lse_val = ((kFp8 ? m : m * sl2) + log2f(l)) * kLn2;
       if (it.partial_slot < 0) {
@@ -694,6 +806,8 @@ cudaError_t attn_tc_configure() {
   e = cudaFuncSetAttribute(attn_tc_kernel<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
 #ifdef SLACK_DIAGNOSTICS
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -702,11 +816,13 @@ cudaError_t attn_tc_configure() {
 }
 
 // p.q_scale != null selects the FP8 instantiation (tm_q / tm_k / tm_v are then byte maps with [128 x 128 B] boxes);
-// p.steps != null the block-sparse one
+// p.steps != null the block-sparse one; p.has_dual the one that serves dual items (the others walk them one by one)
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched) {
   cudaError_t e;
-  if (p.q_scale != nullptr)
+  if (p.has_dual && p.q_scale == nullptr && p.steps == nullptr)
+    e = launch_pdl(attn_tc_kernel<false, false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+  else if (p.q_scale != nullptr)
     e = launch_pdl(attn_tc_kernel<false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   else if (p.steps != nullptr)
     e = launch_pdl(attn_tc_kernel<false, true, false>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);

@@ -66,6 +66,7 @@ struct TcParams {
   int32_t n_heads;
   int32_t page_log2;
   int32_t total_q;
+  int32_t has_dual;     // the plan holds dual items (DevItem::dual): launch the instantiation that serves them
   float scale;          // logits = scale * q.k
 };
 size_t attn_tc_smem_bytes();

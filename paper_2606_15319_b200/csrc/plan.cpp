@@ -127,13 +127,16 @@ void make_candidate(const std::vector<StreamGeom> &order, const std::vector<int3
 constexpr int32_t kMinPiece = 4;
 constexpr bool kAutoPairs = false; // automatic plans use CTA pairs where they pay (see build_plan)
 
+// A row of the balanced plan: one (stream, head, 256-row query block) over the stream's key range, or a DUAL row: two
+// single-tile rows (<= 128 queries each) of the same stream that share a CTA, one per query-tile slot (DevItem::dual).
 struct Row {
   int32_t oi, head, qb, q_rows, tile0, tiles, sink_tiles;
+  int32_t head2 = -1, qb2 = 0, q_rows2 = 0; // companion of a dual row
   double tc;
 };
 
 void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevStream> &ds, int32_t n_heads, int32_t n_cta,
-                   bool pairs, double target_scale, Candidate &c) {
+                   bool pairs, bool allow_dual, double target_scale, Candidate &c) {
   c = Candidate();
   std::vector<Row> rows;
   double total = 0;
@@ -151,29 +154,58 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
         r.tiles = g.tiles;
         r.sink_tiles = g.sink_tiles;
         r.tc = (pairs || r.q_rows > kTileM) ? kTileCost : kTileCost1; // a CTA pair moves at one pace whatever the odd CTA holds
-        total += r.tc * (r.tiles + r.sink_tiles) + kItemOverhead;
         rows.push_back(r);
       }
   }
+  if (allow_dual) { // only where single-tile rows dominate (decode-like batches): the kernel instantiation that serves dual
+                    // items runs ordinary two-tile steps ~5 % slower, so a few 72-row tails among long chunks do not pay
+    size_t singles = 0;
+    for (const Row &r : rows) singles += r.q_rows <= kTileM;
+    allow_dual = 2 * singles >= rows.size();
+  }
+  if (allow_dual) { // single-tile rows of one stream (same key tiles, same step count) pair up, in row order
+    std::vector<Row> merged;
+    std::vector<int32_t> pending(order.size(), -1); // index in `merged` of a single still waiting for a companion
+    for (const Row &r : rows) {
+      if (r.q_rows > kTileM) {
+        merged.push_back(r);
+      } else if (pending[r.oi] >= 0) {
+        Row &a = merged[(size_t)pending[r.oi]];
+        a.head2 = r.head;
+        a.qb2 = r.qb;
+        a.q_rows2 = r.q_rows;
+        a.tc = kTileCost; // two tiles in flight: the pace of a full item
+        pending[r.oi] = -1;
+      } else {
+        pending[r.oi] = (int32_t)merged.size();
+        merged.push_back(r);
+      }
+    }
+    rows.swap(merged);
+  }
+  for (const Row &r : rows) total += r.tc * (r.tiles + r.sink_tiles) + kItemOverhead;
   const double target = target_scale * (total / n_cta) + kItemOverhead;
   std::vector<double> load((size_t)n_cta, 0.0);
   auto emit = [&](const Row &r, int32_t tb, int32_t take, int32_t cta) {
     const DevStream &s = ds[order[r.oi].idx];
-    DevItem it{};
-    it.q_row0 = s.q_row0 + r.qb * kItemRows;
-    it.q_rows = r.q_rows;
-    it.head = r.head;
-    it.pt_off = s.pt_off;
-    it.kv_tile_begin = tb;
-    it.kv_tile_end = tb + take;
-    it.pos_lo = s.pos_lo;
-    it.pos_hi = s.pos_hi;
-    it.partial_slot = -1;
-    it.stream = order[r.oi].idx;
     const bool first_piece = tb == r.tile0;
-    set_sink(it, order[r.oi], s, first_piece);
-    c.items.push_back(it);
-    c.item_cta.push_back(cta);
+    for (int32_t m = 0; m < (r.head2 >= 0 ? 2 : 1); ++m) { // a dual row emits its two items back to back
+      DevItem it{};
+      it.q_row0 = s.q_row0 + (m == 0 ? r.qb : r.qb2) * kItemRows;
+      it.q_rows = m == 0 ? r.q_rows : r.q_rows2;
+      it.head = m == 0 ? r.head : r.head2;
+      it.pt_off = s.pt_off;
+      it.kv_tile_begin = tb;
+      it.kv_tile_end = tb + take;
+      it.pos_lo = s.pos_lo;
+      it.pos_hi = s.pos_hi;
+      it.partial_slot = -1;
+      it.stream = order[r.oi].idx;
+      it.dual = (m == 0 && r.head2 >= 0) ? 1 : 0;
+      set_sink(it, order[r.oi], s, first_piece);
+      c.items.push_back(it);
+      c.item_cta.push_back(cta);
+    }
     load[cta] += r.tc * (take + (first_piece ? r.sink_tiles : 0)) + kItemOverhead;
   };
   // ---- whole rows, earliest-free queue first --------------------------------------------------------------------
@@ -204,18 +236,22 @@ void make_balanced(const std::vector<StreamGeom> &order, const std::vector<DevSt
     first_piece = c.items.size();
   };
   auto close_row = [&]() {
-    const int32_t np = (int32_t)(c.items.size() - first_piece);
+    const Row &r = tail[ti];
+    const int32_t span = r.head2 >= 0 ? 2 : 1; // items per piece
+    const int32_t np = (int32_t)(c.items.size() - first_piece) / span;
     if (np > 1) {
-      const Row &r = tail[ti];
-      DevCombine cb{};
-      cb.q_row0 = c.items[first_piece].q_row0;
-      cb.q_rows = r.q_rows;
-      cb.head = r.head;
-      cb.slot_begin = c.n_slots;
-      cb.n_parts = np;
-      c.combines.push_back(cb);
-      for (int32_t q = 0; q < np; ++q) c.items[first_piece + q].partial_slot = c.n_slots + q;
-      c.n_slots += np;
+      for (int32_t m = 0; m < span; ++m) {
+        const DevItem &i0 = c.items[first_piece + (size_t)m];
+        DevCombine cb{};
+        cb.q_row0 = i0.q_row0;
+        cb.q_rows = i0.q_rows;
+        cb.head = i0.head;
+        cb.slot_begin = c.n_slots;
+        cb.n_parts = np;
+        c.combines.push_back(cb);
+        for (int32_t q = 0; q < np; ++q) c.items[first_piece + (size_t)(q * span + m)].partial_slot = c.n_slots + q;
+        c.n_slots += np;
+      }
     }
     ++ti;
     if (ti < tail.size()) open_row();
@@ -454,7 +490,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     const double scales[] = {1.0, 0.99, 1.01, 0.98, 1.02, 0.97, 1.03, 1.045, 1.06};
     for (double sc : scales) {
       Candidate c;
-      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, sc, c);
+      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, out.kernel_kind == 0 && !fp8, sc, c);
       if (c.objective < best.objective - 1e-9) best = std::move(c);
     }
   }
@@ -487,6 +523,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   }
   // block-sparse bookkeeping: which mask row an item reads and where its compacted step list goes
   for (DevItem &it : out.items) {
+    out.has_dual |= it.dual != 0;
     const DevStream &d = out.streams[it.stream];
     it.mask_row = d.qblock0 + (it.q_row0 - d.q_row0) / kItemRows;
     it.step_off = (int32_t)out.total_steps;

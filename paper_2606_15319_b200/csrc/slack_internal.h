@@ -15,7 +15,7 @@ constexpr int kTileM = 128;    // query rows per MMA tile (UMMA M)
 constexpr int kTileN = 128;    // keys per KV tile (UMMA N of QK^T, K extent of PV); anchored to page slots
 constexpr int kItemRows = 256; // an item carries two query tiles that ping-pong on the tensor pipe
 
-// One planned unit of work as the kernels read it (device copy of slack_work_item plus table offsets). 64 bytes.
+// One planned unit of work as the kernels read it (device copy of slack_work_item plus table offsets). 80 bytes.
 // Key tiles are visited in the order: sink tiles [sink_tile0, sink_tile0 + sink_tiles) with visible positions
 // [sink_lo, sink_hi) ("sink + local"; only the first piece of a row carries them), then the window tiles
 // [kv_tile_begin, kv_tile_end) with visible positions [pos_lo, pos_hi).
@@ -36,8 +36,13 @@ struct DevItem {
   int32_t sink_tiles;
   int32_t mask_row;      // block-sparse: global 256-row query block of the item = row of the block mask (P:88 knob (2))
   int32_t step_off;      // block-sparse: offset of the item's compacted step list (uint16 units) in the sparse workspace
+  int32_t dual;          // 1: this item (<= 128 rows) and the NEXT one of the queue (<= 128 rows, same number of key steps,
+                         // any stream / head) share a CTA: this one takes query-tile slot 0, the next one slot 1, each with
+                         // its own K/V tiles (decode-like chunks; the 72-row tails of long chunks).  Kernels that do not
+                         // implement it (block-sparse, FP8, SIMT) just walk the two items one after the other
+  int32_t pad[3];
 };
-static_assert(sizeof(DevItem) == 64, "DevItem layout");
+static_assert(sizeof(DevItem) == 80, "DevItem layout");
 
 // One output row-block whose key range was cut: the combine kernel merges its partial slots (A4).
 struct DevCombine {
@@ -91,6 +96,7 @@ struct HostPlan {
   std::vector<int32_t> item_cta;     // per item
   std::vector<DevCombine> combines;
   int32_t n_partial_slots = 0;
+  bool has_dual = false;   // some item carries DevItem::dual
   WorkspaceLayout ws;
   // FP8 pools: the attention call quantises Q into the workspace first: codes [total_q][H][128] u8, scales [H][total_q] f32
   size_t q8_off = 0, q8_scale_off = 0;

@@ -52,7 +52,7 @@ def test_every_declared_symbol_is_exported_and_bound():
 def test_struct_sizes_match_header():
     import ctypes as C
     assert C.sizeof(binding.CPool) == 56 and C.sizeof(binding.CStream) == 40
-    assert C.sizeof(binding.CPlanOpts) == 16 and C.sizeof(binding.CWorkItem) == 48
+    assert C.sizeof(binding.CPlanOpts) == 16 and C.sizeof(binding.CWorkItem) == 52
 
 
 def test_host_only_context_has_no_data_path(hctx):
@@ -86,6 +86,11 @@ def check_cover(w, plan, n_cta):
         assert it["kv_tile_begin"] < it["kv_tile_end"]
     ctas = [it["cta"] for it in items]
     assert ctas == sorted(ctas), "items must be stored queue by queue"
+    for a, b in zip(items, items[1:] + [None]):     # dual items: the companion follows in the same queue, same key steps
+        if a["dual"]:
+            assert b is not None and b["cta"] == a["cta"] and not b["dual"]
+            assert a["q_rows"] <= 128 and b["q_rows"] <= 128
+            assert (a["kv_tile_end"] - a["kv_tile_begin"], a["sink_tiles"]) == (b["kv_tile_end"] - b["kv_tile_begin"], b["sink_tiles"])
     slots = [it["partial_slot"] for it in items if it["partial_slot"] >= 0]
     assert sorted(slots) == list(range(plan.num_partial_slots))
     for si, s in enumerate(w.streams):
@@ -154,8 +159,13 @@ def test_plan_cover_and_balance_full_configs(hctx, maker, pairs):
     nq = 148 // pairs
     items = check_cover(w, plan, nq)
     load = np.zeros(nq)
+    companion = False
     for it in items:
-        load[it["cta"]] += (2.0 if (pairs == 2 or it["q_rows"] > 128) else 1.70) * (it["kv_tile_end"] - it["kv_tile_begin"]) + 7.75
+        if companion:                # second member of a dual item: rides in the first one's key steps
+            companion = False
+            continue
+        companion = bool(it["dual"])
+        load[it["cta"]] += (2.0 if (pairs == 2 or it["q_rows"] > 128 or it["dual"]) else 1.70) * (it["kv_tile_end"] - it["kv_tile_begin"]) + 7.75
     assert load.max() <= 1.25 * load.mean() + 40, f"{w.name}: makespan {load.max():.0f} vs ideal {load.mean():.0f}"
 
 
