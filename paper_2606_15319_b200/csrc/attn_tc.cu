@@ -87,6 +87,7 @@ constexpr float kRescaleThreshold8 = 1.0f; // FP8: P = 128 * 2^(z - m) must stay
 // the launch allocates (2048 exactly never gets its last increase granted: the bounded waits trap).  Measured on cfg5:
 // 80 / 208: 1147 TFLOP/s, 72 / 216: 1169 (the softmax path wants ~210 registers: 44 instead of 88 bytes of spills),
 // 64 / 216: 1169, 56 / 224: 1107 and 40 / 232: 1115 (producer / issuer starved), 88 / 208: 1148, 104 / 200: 1133.
+// (The two idle warps cannot hand their share over: registers of warps that exit do not return to the pool.)
 #ifndef SLACK_REG_LOW
 #define SLACK_REG_LOW 72
 #endif
