@@ -278,7 +278,7 @@ def load_peaks():
 
 
 def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2e, want_cpu, want_xfer, sparsity=0.0,
-            sample_clocks=True):
+            sample_clocks=True, dtype=None):
     """One workload: fills 30 layers of pools on the device, times `steps` steps, returns the pieces of the JSON line."""
     import torch
     from paper_2606_15319_b200 import binding, metrics
@@ -290,7 +290,7 @@ def measure(ctx, args, name, steps, warmup, rank, world, local, dist, *, want_e2
     gen = torch.Generator(device=dev)
     gen.manual_seed(777 + rank)
     rnd = lambda *shape: (torch.randn(*shape, device=dev, dtype=torch.float32, generator=gen) * 0.5).to(torch.bfloat16)
-    fp8 = args.dtype == "fp8"
+    fp8 = (dtype or args.dtype) == "fp8"
     pools, qs, kns, vns, outs = [], [], [], [], []
     for l in range(L):
         if fp8:
@@ -597,21 +597,26 @@ def run_ours(args):
     # ---- supplementary blocks (N = 1 only): the other things `metric` / `north_star` name, a few steps each -----------
     others = {}
     if world == 1 and not args.no_others and args.sparsity == 0 and args.workload == "cfg5" and args.dtype == "bf16":
-        for name, why in (("cfg4", "configs[3] mixed streams: chunks/s"), ("cfg3", "configs[2]: the 460 MB append"),
-                          ("cfg5b", "decode-like short chunks: HBM GB/s")):
+        blocks = (("cfg4", "cfg4", "bf16", 0.0, "configs[3] mixed streams: chunks/s"),
+                  ("cfg3", "cfg3", "bf16", 0.0, "configs[2]: the 460 MB append"),
+                  ("cfg5b", "cfg5b", "bf16", 0.0, "decode-like short chunks: HBM GB/s"),
+                  ("cfg5_sparse_0.8", "cfg5", "bf16", 0.8, "block-sparse variant (P:88 knob (2)), selected flops"),
+                  ("cfg5_fp8", "cfg5", "fp8", 0.0, "FP8 pool variant (P:88 knob (4)): peak = 2 x the bf16 burst figure"),
+                  ("cfg5b_fp8", "cfg5b", "fp8", 0.0, "FP8 pool variant, decode-like: GB/s of 1-byte K/V"))
+        for key, name, dt, rho, why in blocks:
             gc.collect()
             torch.cuda.empty_cache()
             o = measure(ctx, args, name, 5, 3, rank, world, local, dist, want_e2e=False, want_cpu=False, want_xfer=False,
-                        sample_clocks=True)
+                        sample_clocks=True, dtype=dt, sparsity=rho)
             rf, ap = o["roofline"], o["append"]
-            others[name] = {"workload": workload_label(args, o["w"], name), "why": why, "steps": 5, "warmup": 3,
-                            "tflops": o["value"], "ms_per_step": o["ms_per_step"], "step_ms": o["step_ms"],
-                            "chunks_per_s_30_layers_1_step": o["chunks_per_s"], "streams": len(o["w"].streams),
-                            "attention": {k: rf.get(k) for k in ("bound", "achieved", "unit", "peak", "frac", "kernel_ms_avg",
-                                                                 "kernel_share_of_step", "tflops", "bytes_per_launch")},
-                            "append": {k: ap.get(k) for k in ("ms_avg", "ms_min", "bytes_per_launch", "GB_per_s", "frac_of_hbm")} if ap else None,
-                            "combine_ms_avg": o["combine"]["ms_avg"] if o["combine"] else None,
-                            "clocks": o["clocks"]}
+            others[key] = {"workload": workload_label(args, o["w"], name), "why": why, "dtype": dt, "sparsity": rho, "steps": 5,
+                           "warmup": 3, "tflops": o["value"], "ms_per_step": o["ms_per_step"], "step_ms": o["step_ms"],
+                           "chunks_per_s_30_layers_1_step": o["chunks_per_s"], "streams": len(o["w"].streams),
+                           "attention": {k: rf.get(k) for k in ("bound", "achieved", "unit", "peak", "frac", "kernel_ms_avg",
+                                                                "kernel_share_of_step", "tflops", "bytes_per_launch")},
+                           "append": {k: ap.get(k) for k in ("ms_avg", "ms_min", "bytes_per_launch", "GB_per_s", "frac_of_hbm")} if ap else None,
+                           "combine_ms_avg": o["combine"]["ms_avg"] if o["combine"] else None,
+                           "clocks": o["clocks"]}
             del o
 
     if dist is not None:
