@@ -314,8 +314,11 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
     } else if (warp == 1) {
       // ============================== MMA issuer ==============================
       uint32_t ring = 0;
-      uint32_t cnt[2] = {0, 0}; // kv steps seen per query tile (parity of S_FULL / P_READY)
-      uint32_t itn[2] = {0, 0}; // items seen per query tile (parity of O_FINAL / O_FREE)
+      // parities of the per-tile barriers, bit i = query tile i (kept in two scalars: indexed arrays would live in local
+      // memory, on the issuer's critical path): steps seen (S_FULL / P_LO / P_READY) and items seen (O_FINAL / O_FREE)
+      uint32_t cnt_par = 0, itn_par = 0;
+      auto cnt_of = [&](int i) { return (cnt_par >> i) & 1u; };
+      auto itn_of = [&](int i) { return (itn_par >> i) & 1u; };
       int n_item = 0;
       auto issue_qk = [&](int i, uint32_t stage) {
         const uint32_t a_base = sQ + i * kTileBytes;
@@ -416,12 +419,12 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
               entry(i, j, 1, stage_v, ph_v);
               mbar_wait(bar(BAR_KV_FULL + stage_v), ph_v, 220 + stage_v, dbg);
               zero_masked_v(i == 0 ? v : vb, j, stage_v);
-              mbar_wait(bar(BAR_P_LO + i), cnt[i] & 1u, 260 + i, dbg);
-              if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
+              mbar_wait(bar(BAR_P_LO + i), cnt_of(i), 260 + i, dbg);
+              if (j == 0) mbar_wait(bar(BAR_O_FREE + i), itn_of(i) ^ 1u, 240 + i, dbg);
               tc_fence_after();
               if (elect_one()) issue_pv(i, stage_v, 0, j > 0);
               __syncwarp();
-              mbar_wait(bar(BAR_P_READY + i), cnt[i] & 1u, 230 + i, dbg);
+              mbar_wait(bar(BAR_P_READY + i), cnt_of(i), 230 + i, dbg);
               if (has_next) {
                 entry(i, j + 1, 0, stage_k, ph_k);
                 mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
@@ -440,8 +443,8 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                 }
               }
               __syncwarp();
-              cnt[i]++;
-              if (!has_next) itn[i]++;
+              cnt_par ^= 1u << i;
+              if (!has_next) itn_par ^= 1u << i;
             }
           }
           ring = r0 + 4u * (uint32_t)Ts;
@@ -495,13 +498,13 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           }
           tc_fence_after();
           for (int i = 0; i < v.nq; ++i) {
-            mbar_wait(bar(BAR_P_LO + i), cnt[i] & 1u, 260 + i, dbg);
-            if (j == 0) mbar_wait(bar(BAR_O_FREE + i), (itn[i] & 1u) ^ 1u, 240 + i, dbg);
+            mbar_wait(bar(BAR_P_LO + i), cnt_of(i), 260 + i, dbg);
+            if (j == 0) mbar_wait(bar(BAR_O_FREE + i), itn_of(i) ^ 1u, 240 + i, dbg);
             tc_fence_after();
             SLACK_TRACE(2, j, 2 + 2 * i);
             if (elect_one()) issue_pv(i, stage_v, 0, j > 0);
             __syncwarp();
-            mbar_wait(bar(BAR_P_READY + i), cnt[i] & 1u, 230 + i, dbg);
+            mbar_wait(bar(BAR_P_READY + i), cnt_of(i), 230 + i, dbg);
             if (has_next && i == 0) mbar_wait(bar(BAR_KV_FULL + stage_k), ph_k, 250 + stage_k, dbg);
             tc_fence_after();
             if (elect_one()) {
@@ -520,8 +523,8 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             }
             __syncwarp();
             SLACK_TRACE(2, j, 3 + 2 * i);
-            cnt[i]++;
-            if (!has_next) itn[i]++;
+            cnt_par ^= 1u << i;
+            if (!has_next) itn_par ^= 1u << i;
           }
         }
         ring = r0 + 2u * (uint32_t)Ts;
