@@ -54,7 +54,7 @@ typedef enum {
   SLACK_EINVAL = 1,       /* malformed descriptors: negative lengths, base >= page_size, short page table, page id out of
                              range, a physical page owned twice in the batch, misaligned (<16 B) pointer, NULL argument */
   SLACK_EUNSUPPORTED = 2, /* valid but not built: head_dim not in {64,128}, page_size not a power of two >= 16; FP8 pools
-                             with head_dim != 128, page_size < 128, force_simt, the block-sparse call or slack_kv_transfer */
+                             with head_dim != 128, page_size < 128, force_simt or the block-sparse call */
   SLACK_ENOMEM = 3,       /* host or device allocation failed, or workspace_bytes too small */
   SLACK_ECUDA = 4,        /* a CUDA runtime/driver call failed, or the context has no device */
   SLACK_ESTALE_PLAN = 5   /* plan does not match the pool shape / dtype passed with it */
@@ -216,7 +216,8 @@ int32_t slack_plan_mask_min_words(const slack_plan_t *plan); /* ceil(max over st
  * only the head partition assigned to the donor worker moves.
  * For each layer l = 0 .. n_layers-1, in order: page src_page_ids[i] of src_pools[l] is copied, bit for bit, into page
  * dst_page_ids[i] of dst_pools[l], heads [head_begin, head_end) only (in the [n_pages][H][P][D] layout a page's head
- * slice is one contiguous run); no other byte of the destination changes.  One kernel per layer on `cuda_stream`
+ * slice is one contiguous run); no other byte of the destination changes.  FP8 pools: the block scales of the moved
+ * (page, head) slices are copied with the codes (a second small kernel per layer).  One kernel per layer on `cuda_stream`
  * (asynchronous: give it a side stream to overlap with compute); if layer_done_events is not NULL, entry l (a
  * cudaEvent_t, may be NULL) is recorded right after layer l's copy, which is what a consumer of layer l waits for.
  * src_pools / dst_pools: HOST arrays of n_layers descriptors; all layers of one side share n_pages, both sides share

@@ -646,9 +646,10 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
   if (!src_pools || !dst_pools || !src_page_ids || !dst_page_ids) return set_err(ctx, SLACK_EINVAL, "NULL argument");
   const slack_pool &s0 = src_pools[0];
   const slack_pool &d0 = dst_pools[0];
-  if (s0.dtype == SLACK_FP8_E4M3) return set_err(ctx, SLACK_EUNSUPPORTED, "slack_kv_transfer: FP8 pools (codes + scales) are not built");
-  if (s0.n_heads <= 0 || s0.head_dim <= 0 || s0.page_size <= 0 || (s0.dtype != SLACK_BF16 && s0.dtype != SLACK_F32))
+  const bool fp8 = s0.dtype == SLACK_FP8_E4M3; // codes move like any other element type; the block scales move with them
+  if (s0.n_heads <= 0 || s0.head_dim <= 0 || s0.page_size <= 0 || (s0.dtype != SLACK_BF16 && s0.dtype != SLACK_F32 && !fp8))
     return set_err(ctx, SLACK_EINVAL, "bad source pool shape / dtype");
+  if (fp8 && s0.page_size % 128 != 0) return set_err(ctx, SLACK_EUNSUPPORTED, "FP8 pools need page_size >= 128");
   if (((size_t)s0.page_size * s0.head_dim * elem_bytes(s0.dtype)) % 16 != 0)
     return set_err(ctx, SLACK_EUNSUPPORTED, "a (page, head) slice must be a multiple of 16 bytes");
   if (head_begin < 0 || head_end > s0.n_heads || head_begin >= head_end)
@@ -692,6 +693,9 @@ slack_status slack_kv_transfer(slack_ctx *ctx, int32_t n_layers, const slack_poo
     e = launch_kv_transfer(src_pools[l].k_pool, src_pools[l].v_pool, dst_pools[l].k_pool, dst_pools[l].v_pool, d_src, d_dst,
                            n_pages, s0.n_heads, s0.head_dim, s0.page_size, elem_bytes(s0.dtype), head_begin, head_end,
                            ctx->sm_count, cs, &ctx->last_launches);
+    if (e == cudaSuccess && fp8)
+      e = launch_kv_scale_transfer(src_pools[l].k_scale, src_pools[l].v_scale, dst_pools[l].k_scale, dst_pools[l].v_scale, d_src, d_dst,
+                                   n_pages, s0.n_heads, s0.page_size, head_begin, head_end, cs, &ctx->last_launches);
     if (e == cudaSuccess && layer_done_events && layer_done_events[l])
       e = cudaEventRecord(reinterpret_cast<cudaEvent_t>(layer_done_events[l]), cs);
   }

@@ -96,6 +96,11 @@ cudaError_t launch_kv_transfer(const void *src_k, const void *src_v, void *dst_k
                                int elem_bytes, int head_begin, int head_end, int sm_count, cudaStream_t st,
                                int *n_launched);
 
+// NEXT-4 for FP8 pools: the scales of the moved (page, head) slices.
+cudaError_t launch_kv_scale_transfer(const float *src_k, const float *src_v, float *dst_k, float *dst_v, const int32_t *d_src_ids,
+                                     const int32_t *d_dst_ids, int n_pages, int n_heads, int page_size, int head_begin,
+                                     int head_end, cudaStream_t st, int *n_launched);
+
 // A4: merge split-KV partials into `out` (bf16) and `lse`.
 cudaError_t launch_combine(const DevCombine *d_combines, int n_combines, const float *ws_o, const float *ws_lse, void *out,
                            float *lse, int n_heads, int head_dim, int total_q, cudaStream_t st, int *n_launched);

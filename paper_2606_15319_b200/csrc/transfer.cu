@@ -48,7 +48,38 @@ kv_transfer_kernel(const uint4 *__restrict__ src_k, const uint4 *__restrict__ sr
   }
 }
 
+// FP8 pools (include/slack.h slack_dtype): the scales of the moved (page, head) slices travel with the codes.  Scales are
+// fp32 [n_pages][H][P / 128]; one thread per (page, head in [h0, h1), block).
+__global__ void __launch_bounds__(kXferThreads)
+kv_scale_transfer_kernel(const float *__restrict__ src_k, const float *__restrict__ src_v, float *__restrict__ dst_k,
+                         float *__restrict__ dst_v, const int32_t *__restrict__ src_ids, const int32_t *__restrict__ dst_ids,
+                         int n_pages, int n_heads, int blocks_per_page, int h0, int h1) {
+  const int per_page = (h1 - h0) * blocks_per_page;
+  const long long n = (long long)n_pages * per_page;
+  for (long long u = (long long)blockIdx.x * kXferThreads + threadIdx.x; u < n; u += (long long)gridDim.x * kXferThreads) {
+    const int pg = (int)(u / per_page), r = (int)(u % per_page);
+    const long long off = (long long)h0 * blocks_per_page + r;
+    const long long s = (long long)src_ids[pg] * n_heads * blocks_per_page + off;
+    const long long d = (long long)dst_ids[pg] * n_heads * blocks_per_page + off;
+    dst_k[d] = src_k[s];
+    dst_v[d] = src_v[s];
+  }
+}
+
 } // namespace
+
+cudaError_t launch_kv_scale_transfer(const float *src_k, const float *src_v, float *dst_k, float *dst_v, const int32_t *d_src_ids,
+                                     const int32_t *d_dst_ids, int n_pages, int n_heads, int page_size, int head_begin,
+                                     int head_end, cudaStream_t st, int *n_launched) {
+  if (n_pages == 0 || head_end <= head_begin) return cudaSuccess;
+  const int bpp = page_size / 128;
+  const long long n = (long long)n_pages * (head_end - head_begin) * bpp;
+  const int grid = (int)((n + kXferThreads - 1) / kXferThreads < 1024 ? (n + kXferThreads - 1) / kXferThreads : 1024);
+  kv_scale_transfer_kernel<<<grid, kXferThreads, 0, st>>>(src_k, src_v, dst_k, dst_v, d_src_ids, d_dst_ids, n_pages, n_heads, bpp,
+                                                           head_begin, head_end);
+  if (n_launched) *n_launched += 1;
+  return cudaGetLastError();
+}
 
 cudaError_t launch_kv_transfer(const void *src_k, const void *src_v, void *dst_k, void *dst_v, const int32_t *d_src_ids,
                                const int32_t *d_dst_ids, int n_pages, int n_heads, int head_dim, int page_size,

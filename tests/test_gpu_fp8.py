@@ -160,3 +160,43 @@ def test_unsupported_combinations(ctx):
     with pytest.raises(binding.SlackError) as e:
         ctx.slack_kv_append(bad, w.streams, binding.to_torch(w.k_new, "bf16", "cuda:0"), binding.to_torch(w.v_new, "bf16", "cuda:0"))
     assert e.value.status == binding.SLACK_EINVAL
+
+
+def test_page_transfer_moves_codes_and_scales(ctx):
+    """NEXT-4 on an FP8 pool: the listed pages' head slices arrive bit for bit, codes AND block scales, nothing else
+    changes; attention through the new page ids gives the same bits as before the move."""
+    w = W.small_ragged(page_size=256)
+    pool = G.make_pool_fp8(w)
+    G.gpu_append_all(ctx, w, pool)
+    out0, lse0, plan0, _ = G.gpu_attention(ctx, w, pool, force_splits=1)
+    s0 = w.streams[0]
+    sp = np.asarray(s0.page_table, dtype=np.int32)
+    dst = G.make_pool_fp8(w)                                     # a second pool of the same shape, NaN-filled
+    dp = np.random.default_rng(3).permutation(w.n_pages)[:sp.size].astype(np.int32)
+    h0, h1 = 0, w.n_heads
+    ctx.slack_kv_transfer([pool], [dst], sp, dp, h0, h1)
+    torch.cuda.synchronize()
+    src_img, dst_img = G.fp8_pool_images(pool), G.fp8_pool_images(dst)
+    want = [np.full_like(a, 0x7F) if a.dtype == np.uint8 else np.full_like(a, np.nan) for a in src_img]
+    oracle.kv_transfer(src_img[0], src_img[1], want[0], want[1], sp, dp, h0, h1)          # codes
+    oracle.kv_transfer(src_img[2], src_img[3], want[2], want[3], sp, dp, h0, h1)          # scales: same slicing rule
+    for g, x in zip(dst_img, want):
+        assert np.array_equal(g, x, equal_nan=True)
+    # a head sub-range moves only that partition (P:660-662)
+    dst2 = G.make_pool_fp8(w)
+    ctx.slack_kv_transfer([pool], [dst2], sp, dp, 1, 2)
+    torch.cuda.synchronize()
+    want2 = [np.full_like(a, 0x7F) if a.dtype == np.uint8 else np.full_like(a, np.nan) for a in src_img]
+    oracle.kv_transfer(src_img[0], src_img[1], want2[0], want2[1], sp, dp, 1, 2)
+    oracle.kv_transfer(src_img[2], src_img[3], want2[2], want2[3], sp, dp, 1, 2)
+    for g, x in zip(G.fp8_pool_images(dst2), want2):
+        assert np.array_equal(g, x, equal_nan=True)
+    # stream 0 re-homed alone into `dst`: same attention bits as inside the original batch (force_splits = 1)
+    import copy
+    s_new = copy.copy(s0)
+    s_new.page_table = dp.copy()
+    w1 = copy.copy(w)
+    w1.streams = [s_new]
+    w1.q = w.q[:s0.q_len]
+    out1, _, _, _ = G.gpu_attention(ctx, w1, dst, force_splits=1)
+    assert np.array_equal(out1, out0[:s0.q_len])
