@@ -791,6 +791,7 @@ slack_status attention_impl(slack_ctx *ctx, const slack_plan_t *plan, const slac
 #endif
   p.dbg_flag = ctx->d_dbg;
   p.n_heads = hp.n_heads;
+  p.head_dim = hp.head_dim;
   int pl2 = 0;
   while ((1 << pl2) < hp.page_size) ++pl2;
   p.page_log2 = pl2;

@@ -1,4 +1,5 @@
-// attn_tc.cu — A3: ragged chunk attention on the 5th-gen tensor cores (tcgen05 + TMEM + TMA), bf16, head_dim 128.
+// attn_tc.cu — A3: ragged chunk attention on the 5th-gen tensor cores (tcgen05 + TMEM + TMA), bf16, head_dim 128 (or 64:
+// the kD = 64 instantiations, same roles and barriers on half-sized tiles; the text below is written for 128).
 //
 // What it computes (include/slack.h; PAPER.md P:21, P:84 chunk attends to cached earlier chunks; P:86 rolling window;
 // P:251 paged pool): for every planned item (stream, head, <=256 query rows, range of 128-key tiles)
@@ -77,7 +78,6 @@ constexpr uint32_t kSmemUsed = kOffScale + kScaleRing * 4;
 constexpr uint32_t kSmemBytes = kSmemUsed + 1024; // slack for manual 1024-byte alignment
 
 constexpr uint32_t kIdescQK = make_idesc_bf16(128, 128, 0, 0);
-constexpr uint32_t kIdescPV = make_idesc_bf16(128, 128, 0, 1);
 constexpr uint32_t kIdescQK8 = make_idesc_e4m3(128, 128, 0, 0);
 constexpr uint32_t kIdescPV8 = make_idesc_e4m3(128, 128, 0, 1);
 constexpr uint32_t kTileBytes8 = 16384;
@@ -151,13 +151,18 @@ __device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
       p.dbg_t[((role) * 64 + (step)) * 8 + (slot)] = (uint32_t)clock64();                                  \
   }
 
-template <bool kTrace, bool kSparse, bool kFp8, bool kDual = false>
+template <bool kTrace, bool kSparse, bool kFp8, bool kDual = false, int kD = 128>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                const __grid_constant__ CUtensorMap tm_v) {
   // dual items (DevItem::dual) are served by a dense bf16 instantiation of their own, launched for plans that hold any:
   // carrying the extra paths costs the issuer warp registers (spills on its critical path: +4.6 % cycles per key step)
-  constexpr bool kDualOk = kDual && !kSparse && !kFp8;
+  constexpr bool kDualOk = kDual && !kSparse && !kFp8 && kD == 128;
+  // head_dim 64 (bf16 only): Q / K / V tiles are ONE 16 KB half ([128 rows][64 d]), Q K^T takes 4 MMAs of K = 16, P V has
+  // N = 64 and O takes the first 64 columns of its TMEM slot; the softmax work per key tile is that of head_dim 128
+  static_assert(kD == 128 || (kD == 64 && !kFp8 && !kDual), "head_dim 64 is served by the bf16 non-dual instantiations");
+  constexpr uint32_t kTileBytesD = 128u * kD * 2u;
+  constexpr uint32_t kIdescPVd = make_idesc_bf16(128, kD, 0, 1);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base + kOffQ;
@@ -246,12 +251,12 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytes8);
             for (int i = 0; i < nq; ++i) tma_load_2d(sQ + i * kTileBytes, &tm_q, bar(BAR_Q_FULL), head * 128, q_row0 + i * kTileM);
           } else {
-            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytes);
+            mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytesD);
             for (int i = 0; i < nq; ++i) {
               const int h_i = (dual && i == 1) ? head_b : head;
               const int r_i = (dual && i == 1) ? q_row0_b : q_row0 + i * kTileM;
-              for (int c = 0; c < 2; ++c)
-                tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), h_i * 128 + c * 64, r_i);
+              for (int c = 0; c < kD / 64; ++c)
+                tma_load_2d(sQ + i * kTileBytes + c * kHalfBytes, &tm_q, bar(BAR_Q_FULL), h_i * kD + c * 64, r_i);
             }
           }
         }
@@ -298,9 +303,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                   mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes8);
                   tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
                 } else {
-                  mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytes);
+                  mbar_expect_tx(bar(BAR_KV_FULL + stage), kTileBytesD);
                   tma_load_2d(sKV + stage * kTileBytes, tm, bar(BAR_KV_FULL + stage), 0, row);
-                  tma_load_2d(sKV + stage * kTileBytes + kHalfBytes, tm, bar(BAR_KV_FULL + stage), 64, row);
+                  if constexpr (kD == 128) tma_load_2d(sKV + stage * kTileBytes + kHalfBytes, tm, bar(BAR_KV_FULL + stage), 64, row);
                 }
               }
               __syncwarp();
@@ -331,7 +336,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                       kIdescQK8, k > 0 ? 1u : 0u);
         } else {
 #pragma unroll
-          for (int k = 0; k < 8; ++k) {
+          for (int k = 0; k < kD / 16; ++k) {
             const uint32_t off = (uint32_t)(k >> 2) * kHalfBytes + (uint32_t)(k & 3) * 32u;
             mma_ss(d, make_smem_desc_sw128(a_base + off, 16, 1024), make_smem_desc_sw128(b_base + off, 16, 1024), kIdescQK,
                    k > 0 ? 1u : 0u);
@@ -354,7 +359,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk) {
             const int k = half * 4 + kk;
-            mma_ts(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 2048u, kHalfBytes, 1024), kIdescPV,
+            mma_ts(d, a + (uint32_t)(k * 8), make_smem_desc_sw128(b_base + (uint32_t)k * 2048u, kHalfBytes, 1024), kIdescPVd,
                    (acc || k > 0) ? 1u : 0u);
           }
         }
@@ -484,7 +489,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             if (c_lo > 0 || c_hi < kTileN) {
               const int n_zero = c_lo + (kTileN - c_hi);
               const uint32_t base = sKV + stage_v * kTileBytes;
-              constexpr int kVecs = kFp8 ? 8 : 16; // 16-byte vectors per key row (FP8: one 128-byte row; bf16: two)
+              constexpr int kVecs = kFp8 ? 8 : kD / 8; // 16-byte vectors per key row (FP8, head_dim 64: one 128-byte row; else two)
               for (int idx = lane; idx < n_zero * kVecs; idx += 32) {
                 int r = idx / kVecs;
                 r = r < c_lo ? r : c_hi + (r - c_lo);
@@ -561,14 +566,14 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         if (local_row < it.q_rows) {
           if (it.partial_slot < 0) {
             uint4 *dst = reinterpret_cast<uint4 *>(reinterpret_cast<__nv_bfloat16 *>(p.out) +
-                                                   ((size_t)(it.q_row0 + local_row) * H + it.head) * 128);
+                                                   ((size_t)(it.q_row0 + local_row) * H + it.head) * kD);
 #pragma unroll
-            for (int e = 0; e < 16; ++e) dst[e] = make_uint4(0u, 0u, 0u, 0u);
+            for (int e = 0; e < kD / 8; ++e) dst[e] = make_uint4(0u, 0u, 0u, 0u);
             if (p.lse != nullptr) p.lse[(size_t)it.head * p.total_q + it.q_row0 + local_row] = -INFINITY;
           } else {
-            float4 *dst = reinterpret_cast<float4 *>(p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * 128);
+            float4 *dst = reinterpret_cast<float4 *>(p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * kD);
 #pragma unroll
-            for (int e = 0; e < 32; ++e) dst[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int e = 0; e < kD / 4; ++e) dst[e] = make_float4(0.f, 0.f, 0.f, 0.f);
             p.ws_lse[(size_t)it.partial_slot * kItemRows + local_row] = -INFINITY;
           }
         }
@@ -705,7 +710,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             m = need ? mx : m;
             l *= alpha;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
+            for (int c = 0; c < kD / 32; ++c) {
               uint32_t r[32];
               tmem_ld32(tO + (uint32_t)(c * 32), r);
               tmem_wait_ld();
@@ -747,9 +752,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       const float lse_val = ((kFp8 ? m : m * sl2) + log2f(l)) * kLn2;
       if (it.partial_slot < 0) {
         __nv_bfloat16 *dst =
-            reinterpret_cast<__nv_bfloat16 *>(p.out) + ((size_t)(it.q_row0 + local_row) * H + it.head) * 128;
+            reinterpret_cast<__nv_bfloat16 *>(p.out) + ((size_t)(it.q_row0 + local_row) * H + it.head) * kD;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < kD / 32; ++c) {
           uint32_t r[32];
           tmem_ld32(tO + (uint32_t)(c * 32), r);
           tmem_wait_ld();
@@ -767,9 +772,9 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         }
         if (valid && p.lse != nullptr) p.lse[(size_t)it.head * p.total_q + it.q_row0 + local_row] = lse_val;
       } else {
-        float *dst = p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * 128;
+        float *dst = p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * kD;
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < kD / 32; ++c) {
           uint32_t r[32];
           tmem_ld32(tO + (uint32_t)(c * 32), r);
           tmem_wait_ld();
@@ -822,6 +827,10 @@ cudaError_t attn_tc_configure() {
   e = cudaFuncSetAttribute(attn_tc_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, false, false, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, true, false, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
 #ifdef SLACK_DIAGNOSTICS
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -834,7 +843,13 @@ cudaError_t attn_tc_configure() {
 cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUtensorMap &tm_k, const CUtensorMap &tm_v,
                            int n_cta, cudaStream_t st, int *n_launched) {
   cudaError_t e;
-  if (p.has_dual && p.q_scale == nullptr && p.steps == nullptr)
+  if (p.head_dim == 64) {
+    if (p.q_scale != nullptr) return cudaErrorInvalidValue; // FP8 pools: head_dim 128 only (the planner refuses the rest)
+    if (p.steps != nullptr)
+      e = launch_pdl(attn_tc_kernel<false, true, false, false, 64>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+    else
+      e = launch_pdl(attn_tc_kernel<false, false, false, false, 64>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+  } else if (p.has_dual && p.q_scale == nullptr && p.steps == nullptr)
     e = launch_pdl(attn_tc_kernel<false, false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   else if (p.q_scale != nullptr)
     e = launch_pdl(attn_tc_kernel<false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);

@@ -46,14 +46,14 @@ cudaError_t launch_attn_simt(int dtype, const void *q, const void *k_pool, const
                              int n_heads, int head_dim, int page_size, float scale, const uint32_t *mask, int mask_words,
                              cudaStream_t st, int *n_launched);
 
-// A3 (tensor-core path, bf16, head_dim 128, page_size >= 128).
+// A3 (tensor-core path: bf16 with head_dim 64 or 128, FP8 with head_dim 128; page_size >= 128).
 struct TcParams {
   const DevItem *items;
   const int32_t *cta_begin;
   const int32_t *page_tables;
-  void *out;            // bf16 [total_q][H][128]
+  void *out;            // bf16 [total_q][H][head_dim]
   float *lse;           // [H][total_q] or null
-  float *ws_o;          // partial outputs [slot][256][128] fp32
+  float *ws_o;          // partial outputs [slot][256][head_dim] fp32
   float *ws_lse;        // partial lse [slot][256]
   float *dbg_s;         // SLACK_DIAGNOSTICS builds: dump of the first S tiles of CTA 0 ([2][128][128] fp32), else null
   uint32_t *dbg_t;      // SLACK_DIAGNOSTICS builds: time-stamp trace (selects the kTrace instantiation), else null
@@ -64,6 +64,7 @@ struct TcParams {
   const float *v_scale;
   const float *q_scale;         // FP8 pools: [H][total_q] scales of the quantised Q (q_quant_kernel)
   int32_t n_heads;
+  int32_t head_dim;     // 128, or 64 (bf16 only: the kD = 64 instantiations)
   int32_t page_log2;
   int32_t total_q;
   int32_t has_dual;     // the plan holds dual items (DevItem::dual): launch the instantiation that serves them

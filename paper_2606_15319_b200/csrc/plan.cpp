@@ -334,7 +334,9 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   const bool fp8 = shape.dtype == SLACK_FP8_E4M3;
   if (fp8 && (shape.head_dim != 128 || shape.page_size < kTileN || opts.force_simt))
     return fail(SLACK_EUNSUPPORTED, "FP8 pools need head_dim 128, page_size >= 128 and the tensor-core kernel");
-  const bool tc_ok = (shape.dtype == SLACK_BF16 || fp8) && shape.head_dim == 128 && shape.page_size >= kTileN;
+  // tensor-core kernel: bf16 with head_dim 64 or 128, FP8 with head_dim 128 (checked above); fp32 pools and pages shorter
+  // than a key tile go to the SIMT kernel
+  const bool tc_ok = (shape.dtype == SLACK_BF16 || fp8) && shape.page_size >= kTileN;
   if (opts.cta_pairs < 0 || opts.cta_pairs > 2) return fail(SLACK_EINVAL, "plan opts: cta_pairs must be 0, 1 or 2");
   out.kernel_kind = (tc_ok && !opts.force_simt) ? 0 : 1;
 
@@ -446,7 +448,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
   // the even CTA and the rest on the odd one, and share every K/V tile.  The plan is then made for n_cta / 2 queues.
   // Pays when most items have more than 128 rows; short chunks (decode-like) keep one CTA per item.
   // cta_pairs: 0 = automatic, 1 = never, 2 = always (needs an even CTA count).
-  if (out.n_cta >= 2 && out.n_cta % 2 == 0 && !fp8) {
+  if (out.n_cta >= 2 && out.n_cta % 2 == 0 && !fp8 && shape.head_dim == 128) {
     bool pairs = opts.cta_pairs == 2;
     if (opts.cta_pairs == 0 && kAutoPairs) {
       int64_t rows = 0, padded = 0;
@@ -490,7 +492,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     const double scales[] = {1.0, 0.99, 1.01, 0.98, 1.02, 0.97, 1.03, 1.045, 1.06};
     for (double sc : scales) {
       Candidate c;
-      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, out.kernel_kind == 0 && !fp8, sc, c);
+      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, out.kernel_kind == 0 && !fp8 && shape.head_dim == 128, sc, c);
       if (c.objective < best.objective - 1e-9) best = std::move(c);
     }
   }

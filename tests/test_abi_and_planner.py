@@ -183,6 +183,11 @@ def test_kernel_kind_selection(hctx):
     assert hctx.slack_plan(_pool(w), w.streams).kernel_kind == 1            # page < 128 -> SIMT
     w = W.small_ragged()
     assert hctx.slack_plan(_pool(w), w.streams, force_simt=1).kernel_kind == 1
+    w = W.small_ragged(head_dim=64)                                         # bf16 head_dim 64: tensor-core kernel, never
+    for pairs in (0, 1, 2):                                                 # CTA pairs, never dual items
+        plan = hctx.slack_plan(_pool(w), w.streams, cta_pairs=pairs)
+        assert plan.kernel_kind == 0 and not any(i["dual"] for i in plan.items())
+    assert hctx.slack_plan(_pool(w), w.streams, force_simt=1).kernel_kind == 1
 
 
 # ------------------------------------------------------------------------------------------------ error behaviour

@@ -121,8 +121,8 @@ def test_sink_plus_local_window_simt(ctx):
 def test_small_ragged_simt_bf16_and_small_pages(ctx):
     res, *_ = run_case(ctx, W.small_ragged(page_size=32))
     assert res["kind"] == 1          # page_size < 128 is served by the SIMT path
-    res, *_ = run_case(ctx, W.small_ragged(head_dim=64))
-    assert res["kind"] == 1          # head_dim 64 likewise
+    res, *_ = run_case(ctx, W.small_ragged(head_dim=64), force_simt=1)
+    assert res["kind"] == 1          # bf16 head_dim 64 on request (by default the tensor-core kernel: test_gpu_d64.py)
 
 
 def test_tensor_core_agrees_with_simt(ctx):
