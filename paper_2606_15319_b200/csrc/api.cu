@@ -565,7 +565,7 @@ slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, c
   if ((st = prof_begin(ctx, 1, cs, &ev_after)) != SLACK_OK) return st;
   if (hp.dtype == SLACK_FP8_E4M3) // k_new / v_new are bf16: the append quantises (quant.cu)
     SLACK_CUDA(ctx, launch_kv_append_fp8(k_new, v_new, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, plan->d_streams,
-                                         hp.n_streams, plan->max_q_len, plan->d_page_tables, hp.n_heads, hp.page_size, cs,
+                                         hp.n_streams, plan->max_q_len, plan->d_page_tables, hp.n_heads, hp.page_size, ctx->d_dbg, cs,
                                          &ctx->last_launches));
   else
     SLACK_CUDA(ctx, launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, plan->d_streams, hp.n_streams, plan->max_q_len,
@@ -613,7 +613,7 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
   cudaError_t e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, cs);
   if (e == cudaSuccess && hp.dtype == SLACK_FP8_E4M3)
     e = launch_kv_append_fp8(k_new, v_new, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, reinterpret_cast<DevStream *>(d),
-                             hp.n_streams, max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.page_size, cs,
+                             hp.n_streams, max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.page_size, ctx->d_dbg, cs,
                              &ctx->last_launches);
   else if (e == cudaSuccess)
     e = launch_kv_append(k_new, v_new, pool->k_pool, pool->v_pool, reinterpret_cast<DevStream *>(d), hp.n_streams, max_q,

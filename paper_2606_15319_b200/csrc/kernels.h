@@ -78,7 +78,8 @@ cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUt
 // NEXT-3 (quant.cu): quantising append into an FP8 pool, and the Q quantiser of the FP8 attention call.
 cudaError_t launch_kv_append_fp8(const void *k_new, const void *v_new, void *k_pool, void *v_pool, float *k_scale, float *v_scale,
                                  const DevStream *d_streams, int n_streams, int max_q_len, const int32_t *d_page_tables,
-                                 int n_heads, int page_size, cudaStream_t st, int *n_launched);
+                                 int n_heads, int page_size, unsigned long long *dbg /* record of a timed-out wait, may be null */,
+                                 cudaStream_t st, int *n_launched);
 cudaError_t launch_q_quant(const void *q, void *q8, float *sq, int total_q, int n_heads, cudaStream_t st, int *n_launched);
 
 // A3 on CTA pairs (attn_tc2.cu, tcgen05 cta_group::2): needs a pair plan (HostPlan::kernel_kind 2, even n_cta) and a K

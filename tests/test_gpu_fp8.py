@@ -64,6 +64,36 @@ def test_append_planned_reappend_and_large_values(ctx):
     assert np.isin(G.fp8_pool_images(pool)[0], (0x7E, 0xFE)).any(), "the case must exercise saturation"
 
 
+def test_append_division_bit_exact_over_extreme_scales(ctx):
+    """code = e4m3(fp32(x) / scale) with the IEEE division of the rule, whatever the magnitudes: every fresh 128-token block
+    (and head) is scaled by its own power of two from 2^-140 (bf16 denormals: a denormal scale) to 2^120, one block holds
+    an infinity, zeros of both signs are sprinkled in, and the 64 tokens that CONTINUE the block started by the earlier
+    chunk are spread over 2^-100 .. 2^100 against its stored scale (quotients far above 448, far below the smallest code,
+    and everything between).  The kernel shares one reciprocal per thread (quant.cu Divider); the oracle divides."""
+    n_blocks = 24
+    w = W.make_workload("fp8_scales", dtype="bf16", n_heads=4, head_dim=128, page_size=256, q_lens=[64 + 128 * n_blocks + 40],
+                        cache_lens=[64], windows=[0], bases=[0], seed=71, amp=0.5, spare_pages=1)
+    rng = np.random.default_rng(72)
+    for name in ("k_new", "v_new"):
+        x = W.bf16_bits_to_f32(getattr(w, name)).astype(np.float64)                  # [Lq, H, D]
+        e_tok = rng.integers(-100, 101, size=(64, w.n_heads, 1))
+        x[:64] *= np.exp2(e_tok)
+        for b in range(n_blocks + 1):
+            e_blk = rng.integers(-140, 121, size=(1, w.n_heads, 1))
+            x[64 + 128 * b: 64 + 128 * (b + 1)] *= np.exp2(e_blk)
+        z = rng.random(x.shape) < 0.01
+        x[z] = np.where(rng.random(int(z.sum())) < 0.5, 0.0, -0.0)
+        x[64 + 128 * 3 + 5, 1, 17] = np.inf                                          # amax = inf -> scale = inf -> codes +-0
+        x[64 + 128 * 3 + 9, 1, 18] = -np.inf                                         # inf / inf -> the NaN code
+        with np.errstate(over="ignore", under="ignore"):
+            setattr(w, name, W.f32_to_bf16_bits(x.astype(np.float32)))
+    pool = G.make_pool_fp8(w)
+    G.gpu_append_all(ctx, w, pool)
+    assert_pool_equals_oracle(w, pool)
+    codes = G.fp8_pool_images(pool)[0]
+    assert np.isin(codes, (0x7E, 0xFE)).any() and np.isin(codes, (0x7F, 0xFF)).any() and (codes == 0x80).any()
+
+
 def test_append_cfg2_full_size_bit_exact(ctx):
     w = W.config2()
     pool = G.make_pool_fp8(w)
