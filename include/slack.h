@@ -117,7 +117,8 @@ typedef struct {
                            applies (debug / cross-check); f32 pools always use it                                */
   int32_t cta_pairs;    /* tensor-core path: 0 = automatic, 1 = one CTA per work item, 2 = CTA pairs (two SMs walk a
                            work item together, 128 query rows each, and share every K/V tile: tcgen05 cta_group::2;
-                           the plan then has sm_count / 2 queues; needs an even sm_count)                       */
+                           the plan then has sm_count / 2 queues; needs an even sm_count; bf16 head_dim 128 only,
+                           one CTA per item otherwise)                                                          */
 } slack_plan_opts;
 
 /* One unit of attention work as planned (inspection only; see slack_plan_get_items). Key tiles are 128 pool slots,
@@ -172,7 +173,9 @@ size_t slack_plan_workspace_bytes(const slack_plan_t *plan); /* device bytes sla
 int32_t slack_plan_num_items(const slack_plan_t *plan);
 int32_t slack_plan_num_partial_slots(const slack_plan_t *plan);
 int32_t slack_plan_kernel_kind(const slack_plan_t *plan);    /* 0 = tcgen05 kernel, one CTA per item; 1 = SIMT kernel;
-                                                                2 = tcgen05 kernel, CTA pairs                      */
+                                                                2 = tcgen05 kernel, CTA pairs.  The tcgen05 kernel
+                                                                serves bf16 pools (head_dim 64 or 128) and FP8 pools
+                                                                with page_size >= 128; the SIMT kernel the rest    */
 /* Copies up to `capacity` planned items (in queue order) to `items`; returns how many were written. */
 int32_t slack_plan_get_items(const slack_plan_t *plan, slack_work_item *items, int32_t capacity);
 
