@@ -16,11 +16,11 @@
 // other tile's P V and next Q K^T.  TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_i is
 // written over the first 64 columns of S_i (two bf16 per 32-bit column).
 //
-// Dual items (DevItem::dual; dense bf16 instantiation only): two single-tile items (<= 128 query rows each: decode-like
+// Dual items (DevItem::dual; dense bf16 and FP8 instantiations of their own): two single-tile items (<= 128 query rows each: decode-like
 // chunks, the 72-row tails of long chunks) of the same number of key steps share the CTA, one per query-tile slot, each
 // with its OWN K/V tiles (ring entries K_a V_a K_b V_b per step): the idle slot of a single-tile item is filled, the key
 // step costs what a two-tile step costs (3250 cycles) instead of 2 x 2755, and an HBM-bound batch keeps twice the
-// bytes in flight per SM.  The other instantiations walk the two items one after the other.
+// bytes in flight per SM.  The other instantiations (block-sparse, head_dim 64) walk the two items one after the other.
 //
 // Block-sparse variant (kSparse, PAPER.md P:88 knob (2) "skips nonselected attention blocks with
 // sparse masks"): an item visits only the key-tile steps listed for it by sparse_steps.cu (the device block mask changes
@@ -157,7 +157,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
                const __grid_constant__ CUtensorMap tm_v) {
   // dual items (DevItem::dual) are served by a dense bf16 instantiation of their own, launched for plans that hold any:
   // carrying the extra paths costs the issuer warp registers (spills on its critical path: +4.6 % cycles per key step)
-  constexpr bool kDualOk = kDual && !kSparse && !kFp8 && kD == 128;
+  constexpr bool kDualOk = kDual && !kSparse && kD == 128;
   // head_dim 64 (bf16 only): Q / K / V tiles are ONE 16 KB half ([128 rows][64 d]), Q K^T takes 4 MMAs of K = 16, P V has
   // N = 64 and O takes the first 64 columns of its TMEM slot; the softmax work per key tile is that of head_dim 128
   static_assert(kD == 128 || (kD == 64 && !kFp8 && !kDual), "head_dim 64 is served by the bf16 non-dual instantiations");
@@ -249,7 +249,11 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         if (elect_one()) {
           if constexpr (kFp8) { // one [128 rows][128 codes] box per query tile
             mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytes8);
-            for (int i = 0; i < nq; ++i) tma_load_2d(sQ + i * kTileBytes, &tm_q, bar(BAR_Q_FULL), head * 128, q_row0 + i * kTileM);
+            for (int i = 0; i < nq; ++i) {
+              const int h_i = (dual && i == 1) ? head_b : head;
+              const int r_i = (dual && i == 1) ? q_row0_b : q_row0 + i * kTileM;
+              tma_load_2d(sQ + i * kTileBytes, &tm_q, bar(BAR_Q_FULL), h_i * 128, r_i);
+            }
           } else {
             mbar_expect_tx(bar(BAR_Q_FULL), (uint32_t)nq * kTileBytesD);
             for (int i = 0; i < nq; ++i) {
@@ -264,11 +268,16 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         for (int j0 = 0; j0 < Ts; j0 += 32) { // 32 steps at a time: each lane looks up the pool row of one step's tile
           const int my_jj = j0 + lane;
           int my_row = 0, my_row_b = 0;
-          [[maybe_unused]] float my_sk = 1.f, my_sv = 1.f;
+          [[maybe_unused]] float my_sk = 1.f, my_sv = 1.f, my_sk_b = 1.f, my_sv_b = 1.f;
           if (dual && my_jj < Ts) {
             const int tile_b = vb.tile_of(my_jj);
             const int page_b = __ldg(p.page_tables + pt_off_b + ((tile_b * kTileN) >> p.page_log2));
             my_row_b = (page_b * H + head_b) * P + ((tile_b * kTileN) & (P - 1));
+            if constexpr (kFp8) {
+              const size_t si = ((size_t)page_b * H + head_b) * (size_t)(P >> 7) + (size_t)(((tile_b * kTileN) & (P - 1)) >> 7);
+              my_sk_b = __ldg(p.k_scale + si);
+              my_sv_b = __ldg(p.v_scale + si);
+            }
           }
           if (my_jj < Ts) {
             const int my_tile = v.tile_of(kSparse ? (int)__ldg(steps + my_jj) : my_jj);
@@ -285,12 +294,18 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             const int row_a = __shfl_sync(0xffffffffu, my_row, j);
             const int row_b = dual ? __shfl_sync(0xffffffffu, my_row_b, j) : 0;
             [[maybe_unused]] float t_sk = 1.f, t_sv = 1.f;
+            [[maybe_unused]] float t_sk_b = 1.f, t_sv_b = 1.f;
             if constexpr (kFp8) {
               t_sk = __shfl_sync(0xffffffffu, my_sk, j);
               t_sv = __shfl_sync(0xffffffffu, my_sv, j);
+              if (dual) {
+                t_sk_b = __shfl_sync(0xffffffffu, my_sk_b, j);
+                t_sv_b = __shfl_sync(0xffffffffu, my_sv_b, j);
+              }
             }
             for (int t = 0; t < (dual ? 2 : 1); ++t) { // dual: K_a V_a K_b V_b
             const int row = t == 0 ? row_a : row_b;
+            if (t == 1) t_sk = t_sk_b, t_sv = t_sv_b;
 #pragma unroll
             for (int kv = 0; kv < 2; ++kv) {
               const uint32_t stage = ring % kStages;
@@ -384,10 +399,11 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
           if (c_lo > 0 || c_hi < kTileN) {
             const int n_zero = c_lo + (kTileN - c_hi);
             const uint32_t base = sKV + stage * kTileBytes;
-            for (int idx = lane; idx < n_zero * 16; idx += 32) {
-              int r = idx >> 4;
+            constexpr int kVecsD = kFp8 ? 8 : 16; // 16-byte vectors per key row
+            for (int idx = lane; idx < n_zero * kVecsD; idx += 32) {
+              int r = idx / kVecsD;
               r = r < c_lo ? r : c_hi + (r - c_lo);
-              const int w = idx & 15;
+              const int w = idx % kVecsD;
               const uint32_t addr = base + (uint32_t)(w >> 3) * kHalfBytes + (uint32_t)r * 128u + (uint32_t)(w & 7) * 16u;
               asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
             }
@@ -557,7 +573,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       const ItemView v = view_of(it);
       const int row_base = dual ? 0 : i * kTileM; // this tile's first row inside ITS item
       [[maybe_unused]] const uint32_t r0 = ring;
-      if constexpr (kFp8) ring += 2u * (uint32_t)v.T; // every role counts the item's tiles, also the one that skips it
+      if constexpr (kFp8) ring += (dual ? 4u : 2u) * (uint32_t)v.T; // every role counts the tiles, also the one that skips the item
       if (!dual && i >= v.nq) continue;
       const int Ts = kSparse ? p.item_steps[k] : v.T;
       const uint16_t *steps = kSparse ? p.steps + it.step_off : nullptr;
@@ -582,7 +598,7 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
       float m = -INFINITY, l = 0.f;
       // FP8: scale of this thread's query row (rows past the end of Q hold garbage that is never stored)
       [[maybe_unused]] float q_sc = 1.f;
-      if constexpr (kFp8) q_sc = __ldg(p.q_scale + (size_t)it.head * p.total_q + min(it.q_row0 + i * kTileM + row, p.total_q - 1));
+      if constexpr (kFp8) q_sc = __ldg(p.q_scale + (size_t)it.head * p.total_q + min(it.q_row0 + row_base + row, p.total_q - 1));
       int j_dense = kSparse ? (int)__ldg(steps) : 0;
       for (int j = 0; j < Ts; ++j) {
         const int jd = j_dense; // dense step index (block-sparse: the next one is fetched a step ahead)
@@ -635,8 +651,10 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         // scaled by 2^7 so that its e4m3 codes use the range up to 128 (x 2 before a lazy rescale) of the format's 448.
         [[maybe_unused]] float cz = sl2, az = 0.f, l_fix = 1.f;
         if constexpr (kFp8) {
-          const float t_sk = ld_shared_f32(sScale + ((r0 + 2u * (uint32_t)j) % kScaleRing) * 4u);
-          const float t_sv = ld_shared_f32(sScale + ((r0 + 2u * (uint32_t)j + 1u) % kScaleRing) * 4u);
+          // ring entry of this tile slot's K tile at step j (dual items: K_a V_a K_b V_b per step)
+          const uint32_t rk = dual ? r0 + 4u * (uint32_t)j + 2u * (uint32_t)i : r0 + 2u * (uint32_t)j;
+          const float t_sk = ld_shared_f32(sScale + (rk % kScaleRing) * 4u);
+          const float t_sv = ld_shared_f32(sScale + ((rk + 1u) % kScaleRing) * 4u);
           cz = sl2 * q_sc * t_sk;
           az = log2f(t_sv);
           l_fix = 0.0078125f / t_sv; // this tile's P sums, taken in units of 128 sv_t, back to plain probabilities
@@ -828,6 +846,8 @@ cudaError_t attn_tc_configure() {
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(attn_tc_kernel<false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<false, false, false, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(attn_tc_kernel<false, true, false, false, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -851,6 +871,8 @@ cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUt
       e = launch_pdl(attn_tc_kernel<false, false, false, false, 64>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   } else if (p.has_dual && p.q_scale == nullptr && p.steps == nullptr)
     e = launch_pdl(attn_tc_kernel<false, false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
+  else if (p.q_scale != nullptr && p.has_dual)
+    e = launch_pdl(attn_tc_kernel<false, false, true, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   else if (p.q_scale != nullptr)
     e = launch_pdl(attn_tc_kernel<false, false, true>, dim3(n_cta), dim3(kTcThreads), kSmemBytes, st, p, tm_q, tm_k, tm_v);
   else if (p.steps != nullptr)

@@ -492,7 +492,7 @@ slack_status build_plan(const slack_pool &shape, int32_t n_streams, const slack_
     const double scales[] = {1.0, 0.99, 1.01, 0.98, 1.02, 0.97, 1.03, 1.045, 1.06};
     for (double sc : scales) {
       Candidate c;
-      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, out.kernel_kind == 0 && !fp8 && shape.head_dim == 128, sc, c);
+      make_balanced(order, out.streams, shape.n_heads, n_queues, out.kernel_kind == 2, out.kernel_kind == 0 && shape.head_dim == 128, sc, c);
       if (c.objective < best.objective - 1e-9) best = std::move(c);
     }
   }

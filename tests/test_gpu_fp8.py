@@ -176,6 +176,17 @@ def test_cfg2_full_size_fp8_sampled_rows(ctx):
     assert np.isfinite(out).all()
 
 
+def test_cfg5b_shape_fp8_dual_items_full_output(ctx):
+    """The decode-like supplementary config's shape (72-query chunks over 8190 keys, 12 heads, P = 256) with 12 streams (the
+    oracle dequantises the whole pool image in fp64: 64 streams would need 13 GB), default launch configuration: the plan
+    pairs the heads of a stream into dual items; every output row against the FP8 oracle."""
+    w = W.config5b(n_streams=12)
+    res, out, want = run_fp8(ctx, w)
+    pool = G.make_pool_fp8(w)
+    items = ctx.slack_plan(pool, w.streams).items()
+    assert sum(i["dual"] for i in items) >= len(items) // 4
+
+
 def test_unsupported_combinations(ctx):
     w = W.small_ragged()
     pool = G.make_pool_fp8(w)
@@ -230,3 +241,64 @@ def test_page_transfer_moves_codes_and_scales(ctx):
     w1.q = w.q[:s0.q_len]
     out1, _, _, _ = G.gpu_attention(ctx, w1, dst, force_splits=1)
     assert np.array_equal(out1, out0[:s0.q_len])
+
+
+# ------------------------------------------------------------------------------------------------ dual items on FP8 pools
+def _decode_like(seed, n=10, heads=4, page_size=128):
+    """Many short chunks (1..128 queries) over ragged caches, some windowed, bases anywhere in the first page."""
+    rng = np.random.default_rng(seed)
+    q = [int(x) for x in rng.integers(1, 129, size=n)]
+    c = [int(x) for x in rng.integers(0, 1500, size=n)]
+    wdw = [0 if i % 3 else 700 for i in range(n)]
+    b = [int(x) for x in rng.integers(0, page_size, size=n)]
+    return W.make_workload("decode_like_fp8", dtype="bf16", n_heads=heads, head_dim=128, page_size=page_size, q_lens=q,
+                           cache_lens=c, windows=wdw, bases=b, seed=seed, amp=0.5, spare_pages=2)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+@pytest.mark.parametrize("sm_count", [0, 8, 3])
+def test_decode_like_batches_use_dual_items_fp8(ctx, seed, sm_count):
+    """Two single-tile items share a CTA on FP8 pools too (each tile slot with its own K/V codes AND its own tile scales)."""
+    w = _decode_like(seed)
+    res, *_ = run_fp8(ctx, w, sm_count=sm_count)
+    pool = G.make_pool_fp8(w)
+    items = ctx.slack_plan(pool, w.streams, sm_count=sm_count).items()
+    assert sum(i["dual"] for i in items) >= len(items) // 4, "short chunks should pair up"
+
+
+def test_dual_items_fp8_split_rows_sinks_and_unequal_scales(ctx):
+    """Few queues, long caches: dual rows are cut into pieces; the two members' key tiles carry scales 64 x apart."""
+    w = W.make_workload("decode_long_fp8", dtype="bf16", n_heads=4, head_dim=128, page_size=256, q_lens=[72, 100, 1, 128],
+                        cache_lens=[5000, 5000, 3000, 2500], windows=[0, 4000, 0, 0], bases=[3, 0, 255, 17],
+                        sink_lens=[0, 200, 0, 0], seed=9, amp=0.5, spare_pages=1)
+    for h in range(w.n_heads):                           # heads pair up inside a stream: give each head its own magnitude
+        f = np.float32(8.0 ** (h - 1))
+        for arr in [w.k_new, w.v_new] + list(w.k_prior) + list(w.v_prior):
+            arr[:, h] = W.f32_to_bf16_bits(W.bf16_bits_to_f32(arr[:, h]) * f)
+    w.q = W.f32_to_bf16_bits(W.bf16_bits_to_f32(w.q) * np.float32(0.25))     # keep the logits moderate under the larger K
+    # |out| scales with V (x 64 on the last head, whose 16 x larger logits rest on a few keys: the peaky-row bar 8e-2 x 64);
+    # rel-Fro binds, and a tile scale taken from the wrong member would be off by 8 x or more
+    tol = dict(TOL, max_abs_tol=5.0)
+    res, *_ = run_fp8(ctx, w, tol=tol, sm_count=12)
+    pool = G.make_pool_fp8(w)
+    items = ctx.slack_plan(pool, w.streams, sm_count=12).items()
+    assert any(i["dual"] and i["partial_slot"] >= 0 for i in items)
+
+
+def test_dual_fp8_repeated_launches_are_bit_identical(ctx):
+    w = _decode_like(6)
+    pool = G.make_pool_fp8(w)
+    G.gpu_append_all(ctx, w, pool)
+    plan = ctx.slack_plan(pool, w.streams)
+    assert any(i["dual"] for i in plan.items())
+    q = binding.to_torch(w.q, w.dtype, "cuda:0")
+    ws = torch.full((max(plan.workspace_bytes, 16),), 0xFF, dtype=torch.uint8, device="cuda:0")
+    ref = None
+    for _ in range(20):
+        out = torch.full_like(q, float("nan"))
+        ws.fill_(0xFF)
+        ctx.slack_chunk_attention(plan, pool, q, out, w.scale, workspace=ws)
+        torch.cuda.synchronize()
+        o = out.view(torch.int16).cpu().numpy()
+        ref = o if ref is None else ref
+        assert np.array_equal(o, ref)
