@@ -253,6 +253,24 @@ slack_status make_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t
   return SLACK_OK;
 }
 
+// bf16 rows [rows][cols] read in plain (unswizzled) boxes of 128 rows x 128 elements: the FP8 append stages the 256-byte
+// (token, head) rows of one key block with a single TMA instruction
+slack_status make_rows_map(slack_ctx *ctx, CUtensorMap *m, const void *base, uint64_t cols, uint64_t rows) {
+  const cuuint64_t dims[2] = {cols, rows};
+  const cuuint64_t strides[1] = {cols * 2};
+  const cuuint32_t box[2] = {128u, 128u};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    char buf[128];
+    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    return set_err(ctx, SLACK_ECUDA, buf);
+  }
+  return SLACK_OK;
+}
+
 int elem_bytes(int dtype) { return dtype == SLACK_BF16 ? 2 : dtype == SLACK_FP8_E4M3 ? 1 : 4; }
 
 // The first launches that use a plan wait, on the device, for its upload; every stream that reads the tables is noted
@@ -563,8 +581,13 @@ slack_status slack_kv_append_planned(slack_ctx *ctx, const slack_plan_t *plan, c
   if ((st = plan_in_use(ctx, plan, cs)) != SLACK_OK) return st;
   cudaEvent_t ev_after;
   if ((st = prof_begin(ctx, 1, cs, &ev_after)) != SLACK_OK) return st;
+  CUtensorMap tm_kn, tm_vn;
+  if (hp.dtype == SLACK_FP8_E4M3) {
+    if ((st = make_rows_map(ctx, &tm_kn, k_new, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
+    if ((st = make_rows_map(ctx, &tm_vn, v_new, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q)) != SLACK_OK) return st;
+  }
   if (hp.dtype == SLACK_FP8_E4M3) // k_new / v_new are bf16: the append quantises (quant.cu)
-    SLACK_CUDA(ctx, launch_kv_append_fp8(k_new, v_new, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, plan->d_streams,
+    SLACK_CUDA(ctx, launch_kv_append_fp8(tm_kn, tm_vn, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, plan->d_streams,
                                          hp.n_streams, plan->max_q_len, plan->d_page_tables, hp.n_heads, hp.page_size, ctx->d_dbg, cs,
                                          &ctx->last_launches));
   else
@@ -610,9 +633,18 @@ slack_status slack_kv_append(slack_ctx *ctx, const slack_pool *pool, int32_t n_s
   memcpy(h + b_streams, hp.page_tables.data(), hp.page_tables.size() * sizeof(int32_t));
   int max_q = 0;
   for (const DevStream &s : hp.streams) max_q = s.q_len > max_q ? s.q_len : max_q;
+  CUtensorMap tm_kn, tm_vn;
+  if (hp.dtype == SLACK_FP8_E4M3) {
+    slack_status ms = make_rows_map(ctx, &tm_kn, k_new, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q);
+    if (ms == SLACK_OK) ms = make_rows_map(ctx, &tm_vn, v_new, (uint64_t)hp.n_heads * hp.head_dim, (uint64_t)hp.total_q);
+    if (ms != SLACK_OK) {
+      ctx->arena.free_now(blk);
+      return ms;
+    }
+  }
   cudaError_t e = cudaMemcpyAsync(d, h, total, cudaMemcpyHostToDevice, cs);
   if (e == cudaSuccess && hp.dtype == SLACK_FP8_E4M3)
-    e = launch_kv_append_fp8(k_new, v_new, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, reinterpret_cast<DevStream *>(d),
+    e = launch_kv_append_fp8(tm_kn, tm_vn, pool->k_pool, pool->v_pool, pool->k_scale, pool->v_scale, reinterpret_cast<DevStream *>(d),
                              hp.n_streams, max_q, reinterpret_cast<int32_t *>(d + b_streams), hp.n_heads, hp.page_size, ctx->d_dbg, cs,
                              &ctx->last_launches);
   else if (e == cudaSuccess)

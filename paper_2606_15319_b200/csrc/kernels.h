@@ -76,7 +76,8 @@ cudaError_t launch_attn_tc(const TcParams &p, const CUtensorMap &tm_q, const CUt
                            int n_cta, cudaStream_t st, int *n_launched);
 
 // NEXT-3 (quant.cu): quantising append into an FP8 pool, and the Q quantiser of the FP8 attention call.
-cudaError_t launch_kv_append_fp8(const void *k_new, const void *v_new, void *k_pool, void *v_pool, float *k_scale, float *v_scale,
+// tm_k_new / tm_v_new: unswizzled bf16 maps over K_new / V_new [sum Lq][H * 128] with 128 x 128 boxes (api.cu make_rows_map)
+cudaError_t launch_kv_append_fp8(const CUtensorMap &tm_k_new, const CUtensorMap &tm_v_new, void *k_pool, void *v_pool, float *k_scale, float *v_scale,
                                  const DevStream *d_streams, int n_streams, int max_q_len, const int32_t *d_page_tables,
                                  int n_heads, int page_size, unsigned long long *dbg /* record of a timed-out wait, may be null */,
                                  cudaStream_t st, int *n_launched);

@@ -6,7 +6,7 @@
 //   kv_append_fp8_kernel  A1 for FP8 pools: one CTA per (key block of 128 slots, head, stream x {K, V}); a block whose
 //                         first held token this append writes gets its scale from the tokens written, any other
 //                         block keeps the stored scale.  The block's rows (<= 128 x 256 B) are staged in shared memory by
-//                         bulk copies (cp.async.bulk) and read from there for the amax and for the conversion:
+//                         one TMA box load (cp.async.bulk.tensor) and read from there for the amax and for the conversion:
 //                         HBM-bound, 2 * Lq * H * D * 2 B read once, half of that written.
 //                         The per-element division shares one reciprocal per thread (Divider: same bits as __fdiv_rn).
 //   q_quant_kernel        Q of an attention call -> codes [sum Lq][H][128] + scales [H][sum Lq] in the workspace;
@@ -89,12 +89,12 @@ __device__ __forceinline__ float warp_max(float v) {
 }
 
 __global__ void __launch_bounds__(kQuantThreads, 6)
-kv_append_fp8_kernel(const uint4 *__restrict__ k_new, const uint4 *__restrict__ v_new, uint2 *__restrict__ k_pool,
+kv_append_fp8_kernel(const __grid_constant__ CUtensorMap tm_k_new, const __grid_constant__ CUtensorMap tm_v_new, uint2 *__restrict__ k_pool,
                      uint2 *__restrict__ v_pool, float *__restrict__ k_scale, float *__restrict__ v_scale,
                      const DevStream *__restrict__ streams, const int32_t *__restrict__ page_tables, int n_heads, int page_log2,
                      unsigned long long *dbg) {
-  // the block's token rows (<= 128 x 256 B), staged by bulk copies: no registers are tied up while they are in flight,
-  // so six CTAs per SM keep ~190 KB of loads outstanding
+  // the block's token rows (<= 128 x 256 B), staged by ONE TMA box load: no registers are tied up while they are in
+  // flight, so six CTAs per SM keep ~190 KB of loads outstanding
   __shared__ alignas(128) uint4 tile[128 * 16];
   __shared__ alignas(8) unsigned long long mbar;
   __shared__ float red[kQuantThreads / 32];
@@ -113,15 +113,17 @@ kv_append_fp8_kernel(const uint4 *__restrict__ k_new, const uint4 *__restrict__ 
   const int kb = (s.app_pos0 >> 7) + blockIdx.x; // key block in the stream's position space
   const int p_first = max(kb << 7, s.app_pos0), p_last = min((kb << 7) + 128, s.app_pos0 + s.q_len); // positions written here
   if (p_first >= p_last) return;
-  const uint4 *src = is_v ? v_new : k_new;
   uint2 *pool = is_v ? v_pool : k_pool;
   float *scales = is_v ? v_scale : k_scale;
   const int n_tok = p_last - p_first;
   const int tok0 = p_first - s.app_pos0; // chunk-local index of the first token written here
-  // A token row of one head is 128 bf16 = 256 contiguous bytes of the source, H rows apart from the next token's
-  if (threadIdx.x == 0) ptx::mbar_expect_tx(bar, (uint32_t)n_tok * 256u);
-  if ((int)threadIdx.x < n_tok)
-    ptx::bulk_load(ptx::smem_u32(tile + threadIdx.x * 16), src + ((size_t)(s.q_row0 + tok0 + threadIdx.x) * n_heads + h) * 16, 256u, bar);
+  // A token row of one head is 128 bf16 = 256 contiguous bytes of the source, H rows apart from the next token's: a box of
+  // 128 rows x 128 elements at (column h * 128, row = first token).  Rows past the tokens this CTA writes (the next
+  // stream's, or zero fill past the end of the array) land in the tile and are not used.
+  if (threadIdx.x == 0) {
+    ptx::mbar_expect_tx(bar, 128u * 256u);
+    ptx::tma_load_2d(ptx::smem_u32(tile), is_v ? &tm_v_new : &tm_k_new, bar, h * 128, s.q_row0 + tok0);
+  }
   const int page = page_tables[s.pt_off + ((kb << 7) >> page_log2)];
   const int blocks_per_page = 1 << (page_log2 - 7);
   float *scale_ptr = scales + ((size_t)page * n_heads + h) * blocks_per_page + (((kb << 7) & ((1 << page_log2) - 1)) >> 7);
@@ -186,7 +188,7 @@ q_quant_kernel(const uint2 *__restrict__ q, uint32_t *__restrict__ q8, float *__
 
 } // namespace
 
-cudaError_t launch_kv_append_fp8(const void *k_new, const void *v_new, void *k_pool, void *v_pool, float *k_scale, float *v_scale,
+cudaError_t launch_kv_append_fp8(const CUtensorMap &tm_k_new, const CUtensorMap &tm_v_new, void *k_pool, void *v_pool, float *k_scale, float *v_scale,
                                  const DevStream *d_streams, int n_streams, int max_q_len, const int32_t *d_page_tables,
                                  int n_heads, int page_size, unsigned long long *dbg, cudaStream_t st, int *n_launched) {
   if (n_streams == 0 || max_q_len == 0) return cudaSuccess;
@@ -198,7 +200,7 @@ cudaError_t launch_kv_append_fp8(const void *k_new, const void *v_new, void *k_p
   for (int s0 = 0; s0 < n_streams && e == cudaSuccess; s0 += kMaxZ / 2) {
     const int ns = n_streams - s0 < kMaxZ / 2 ? n_streams - s0 : kMaxZ / 2;
     e = launch_pdl(kv_append_fp8_kernel, dim3(max_blocks, n_heads, 2 * ns), dim3(kQuantThreads), 0, st,
-                   reinterpret_cast<const uint4 *>(k_new), reinterpret_cast<const uint4 *>(v_new), reinterpret_cast<uint2 *>(k_pool),
+                   tm_k_new, tm_v_new, reinterpret_cast<uint2 *>(k_pool),
                    reinterpret_cast<uint2 *>(v_pool), k_scale, v_scale, d_streams + s0, d_page_tables, n_heads, pl2, dbg);
     if (n_launched) *n_launched += 1;
   }
