@@ -189,6 +189,24 @@ slack_status slack_chunk_attention(slack_ctx *ctx, const slack_plan_t *plan, con
                                    void *out, float *lse, float scale, void *workspace, size_t workspace_bytes,
                                    void *cuda_stream);
 
+/* ---- A3 + A4 without a caller workspace ------------------------------------------------------------------------ */
+/* For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): slack_chunk_attention with the workspace in a static device array inside the library instead of an
+ * argument.  Same arguments, preconditions, kernels and results otherwise (dense attention; bit-identical output).
+ * LIMIT: slack_plan_workspace_bytes(plan) <= SLACK_STATIC_WORKSPACE_BYTES (32 MiB: the automatic plans of BASELINE.json
+ * configs[1]-[4] need 0-26 MB), else SLACK_ENOMEM with a message and nothing is launched.  Every GPU that loads the
+ * library holds those 32 MiB until the process exits.  The call itself allocates and frees nothing (no cudaMalloc /
+ * cudaFree, no event or stream creation; launches are not recorded by slack_profile_enable).
+ * SHARING: every call on a device uses the same array, which keeps the previous call's contents; nothing in it has to be
+ * cleared (each call writes every byte it later reads), but two calls that overlap on the GPU - different streams,
+ * different contexts or threads, the same device - RACE on it: order them (one stream, or events).
+ * slack_static_workspace_init resolves the array's device address for ctx's device (once per device; the attention call
+ * does the same on first use) and reports the limit; call it at set-up, e.g. before a stream capture begins. */
+#define SLACK_STATIC_WORKSPACE_BYTES (32u << 20)
+slack_status slack_static_workspace_init(slack_ctx *ctx, size_t *max_bytes /* may be NULL */);
+slack_status slack_chunk_attention_static(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q,
+                                          void *out, float *lse, float scale, void *cuda_stream);
+
 /* ---- A3, block-sparse variant -------------------------------------------------------------- */
 /* PAPER.md P:88 knob (2): "skips nonselected attention blocks with sparse masks", controlled by the attention sparsity
  * rho in {0, .6, .7, .8, .9}.  The block-SELECTION rule is Light Forcing's and not part of this path:

@@ -66,6 +66,8 @@ SYMBOLS = {
     "slack_plan_kernel_kind": (C.c_int32, [_VP]),
     "slack_plan_get_items": (C.c_int32, [_VP, C.POINTER(CWorkItem), C.c_int32]),
     "slack_chunk_attention": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP, C.c_size_t, _VP]),
+    "slack_chunk_attention_static": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP]),
+    "slack_static_workspace_init": (C.c_int, [_VP, C.POINTER(C.c_size_t)]),
     "slack_chunk_attention_sparse": (C.c_int, [_VP, _VP, C.POINTER(CPool), _VP, _VP, _VP, C.c_float, _VP, C.c_int32, _VP,
                                               C.c_size_t, _VP]),
     "slack_plan_sparse_workspace_bytes": (C.c_size_t, [_VP]),
@@ -265,6 +267,17 @@ class Context:
         ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
         self._check(self.lib.slack_chunk_attention(self.handle, plan.handle, C.byref(pool.c), _ptr(q), _ptr(out), _ptr(lse),
                                                    C.c_float(scale), _ptr(workspace), ws_bytes, _cuda_stream(stream)))
+
+    def slack_static_workspace_init(self) -> int:
+        """Resolves the static workspace of this context's device; returns its size (the limit) in bytes."""
+        n = C.c_size_t(0)
+        self._check(self.lib.slack_static_workspace_init(self.handle, C.byref(n)))
+        return int(n.value)
+
+    def slack_chunk_attention_static(self, plan: Plan, pool: Pool, q, out, scale: float, lse=None, stream=None) -> None:
+        """slack_chunk_attention with the library's static workspace (no allocation; include/slack.h for the limit)."""
+        self._check(self.lib.slack_chunk_attention_static(self.handle, plan.handle, C.byref(pool.c), _ptr(q), _ptr(out),
+                                                          _ptr(lse), C.c_float(scale), _cuda_stream(stream)))
 
     def slack_chunk_attention_sparse(self, plan: Plan, pool: Pool, q, out, scale: float, block_mask, lse=None,
                                      workspace=None, stream=None) -> None:

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -875,6 +876,76 @@ slack_status slack_chunk_attention_sparse(slack_ctx *ctx, const slack_plan_t *pl
   if (!ctx) return SLACK_EINVAL;
   if (!block_mask) return set_err(ctx, SLACK_EINVAL, "block_mask NULL (use slack_chunk_attention for dense attention)");
   return attention_impl(ctx, plan, pool, q, out, lse, scale, block_mask, mask_words, workspace, workspace_bytes, cuda_stream);
+}
+
+} // extern "C"
+
+/* ------------------------------------------------------------------------------- attention without a caller workspace */
+// slack_chunk_attention_static: the split-KV partials (and the FP8 path's quantised Q) live in ONE file-scope device array
+// instead of a caller-provided workspace, for callers that may not allocate (CUDA graph capture, tight serving loops).
+// Every GPU that loads libslack.so holds the array's SLACK_STATIC_WORKSPACE_BYTES until the process exits.
+namespace {
+
+static __device__ __align__(256) unsigned char g_static_scratch[SLACK_STATIC_WORKSPACE_BYTES];
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the kernels get the address that
+// cudaGetSymbolAddress reports, looked up once per device with that device current.
+constexpr int kMaxDevices = 64;
+std::mutex g_scratch_mu;
+void *g_scratch_ptr[kMaxDevices] = {};
+
+slack_status static_scratch(slack_ctx *ctx, void **ptr) {
+  slack_status st = ensure_device(ctx); // makes ctx->device the current device
+  if (st != SLACK_OK) return st;
+  if (ctx->device >= kMaxDevices) return set_err(ctx, SLACK_EUNSUPPORTED, "static workspace: device ordinal >= 64");
+  std::lock_guard<std::mutex> lock(g_scratch_mu);
+  if (!g_scratch_ptr[ctx->device]) {
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess) return cuda_err(ctx, e, "cudaGetSymbolAddress(static workspace)");
+    if (!p || !aligned(p, 256)) return set_err(ctx, SLACK_ECUDA, "static workspace: unexpected device address");
+    g_scratch_ptr[ctx->device] = p;
+  }
+  *ptr = g_scratch_ptr[ctx->device];
+  return SLACK_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+slack_status slack_static_workspace_init(slack_ctx *ctx, size_t *max_bytes) {
+  if (!ctx) return SLACK_EINVAL;
+  if (max_bytes) *max_bytes = (size_t)SLACK_STATIC_WORKSPACE_BYTES;
+  void *p = nullptr;
+  return static_scratch(ctx, &p);
+}
+
+slack_status slack_chunk_attention_static(slack_ctx *ctx, const slack_plan_t *plan, const slack_pool *pool, const void *q,
+                                          void *out, float *lse, float scale, void *cuda_stream) {
+  if (!ctx) return SLACK_EINVAL;
+  ctx->last_launches = 0;
+  if (!plan) return set_err(ctx, SLACK_EINVAL, "plan NULL");
+  const size_t need = plan->hp.ws.total;
+  if (need > (size_t)SLACK_STATIC_WORKSPACE_BYTES) {
+    char buf[256];
+    snprintf(buf, sizeof buf,
+             "slack_chunk_attention_static: the plan needs %zu bytes of workspace, the static workspace holds %zu "
+             "(SLACK_STATIC_WORKSPACE_BYTES); use slack_chunk_attention with a caller-provided workspace",
+             need, (size_t)SLACK_STATIC_WORKSPACE_BYTES);
+    return set_err(ctx, SLACK_ENOMEM, buf);
+  }
+  void *ws = nullptr;
+  slack_status st = static_scratch(ctx, &ws);
+  if (st != SLACK_OK) return st;
+  // the per-launch profiling of slack_profile_enable creates events on demand: not on this path
+  const int prof_mask = ctx->prof_mask;
+  ctx->prof_mask = 0;
+  // nothing in the workspace has to start at zero: every byte the combine kernel (or the FP8 attention kernel) reads
+  // was written earlier in this same call (partial outputs + lse of every planned piece; the quantised Q)
+  st = attention_impl(ctx, plan, pool, q, out, lse, scale, nullptr, 0, ws, (size_t)SLACK_STATIC_WORKSPACE_BYTES, cuda_stream);
+  ctx->prof_mask = prof_mask;
+  return st;
 }
 
 } // extern "C"
