@@ -176,6 +176,26 @@ def test_plan_is_deterministic_and_layer_invariant(hctx):
     assert a == b
 
 
+def test_static_workspace_entry_point_needs_a_device(hctx):
+    """slack_chunk_attention_static / slack_static_workspace_init (no-allocation variant): like every data call, refused by
+    a host-only context; the size check against SLACK_STATIC_WORKSPACE_BYTES comes first and needs no device."""
+    w = W.small_ragged(page_size=256)
+    plan = hctx.slack_plan(_pool(w), w.streams, force_splits=3)
+    assert 0 < plan.workspace_bytes <= (32 << 20)
+    with pytest.raises(binding.SlackError) as e:
+        hctx.slack_static_workspace_init()
+    assert e.value.status == binding.SLACK_ECUDA
+    with pytest.raises(binding.SlackError) as e:
+        hctx.slack_chunk_attention_static(plan, _pool(w), None, None, w.scale)
+    assert e.value.status == binding.SLACK_ECUDA
+    w = _descr_only(W.config3)
+    big = hctx.slack_plan(_pool(w), w.streams, force_splits=3)
+    assert big.workspace_bytes > (32 << 20)
+    with pytest.raises(binding.SlackError) as e:
+        hctx.slack_chunk_attention_static(big, _pool(w), None, None, w.scale)
+    assert e.value.status == binding.SLACK_ENOMEM and "static workspace" in str(e.value)
+
+
 def test_kernel_kind_selection(hctx):
     w = W.config1()
     assert hctx.slack_plan(_pool(w), w.streams).kernel_kind == 1            # f32 -> SIMT
