@@ -141,6 +141,62 @@ __device__ __forceinline__ ItemView uniform_view_of(const DevItem &it) {
   return v;
 }
 
+// Epilogue stores of one warp: rows [row0, row0 + 32) of the item (those below q_rows are written), O / l as bf16 (final
+// output; `base` = the item's first output row, `stride` elements between rows) or fp32 (split-KV partial).
+// O leaves TMEM in the 16x256b fragment layout (a quad of lanes owns 8 consecutive columns of a row) and is transposed
+// inside the quads, so that a store instruction writes 64-byte runs of 8 rows instead of 16 bytes of 32 rows: rows are
+// 256 B .. 3 KB apart in memory, and 32 lines per store instruction kept the LSU busy for ~8000 cycles per item.
+// Not inlined: the hot loop's register allocation must not see this code (8 bytes more of spills cost it 1.4 %).
+template <int kD>
+__device__ __noinline__ void store_o(uint32_t tO, float inv_l, int lane, int row0, int q_rows, bool final_out, void *base, size_t stride) {
+  const int fg = lane >> 2, fc = lane & 3;
+#pragma unroll
+  for (int half = 0; half < 2; ++half) {
+#pragma unroll
+    for (int cb = 0; cb < kD / 64; ++cb) {
+      uint32_t r[32];
+      tmem_ld_16x256b_x8(tO + ((uint32_t)(16 * half) << 16) + (uint32_t)(cb * 64), r);
+      tmem_wait_ld();
+#pragma unroll
+      for (int rs = 0; rs < 2; ++rs) {
+        const int wr = 16 * half + 8 * rs + fg; // row inside the warp's 32 (= the lane that owns it: its 1 / l)
+        const float inv = __shfl_sync(0xffffffffu, inv_l, wr);
+        const int lr = row0 + wr;
+        const bool ok = lr < q_rows;
+#pragma unroll
+        for (int mm = 0; mm < 2; ++mm) {                // column groups 4 mm .. 4 mm + 3 of the 64-column block
+          const int col = cb * 64 + 8 * (4 * mm + fc); // after the transpose: this lane's 8 columns
+          if (final_out) {
+            uint32_t a[4];
+#pragma unroll
+            for (int n = 0; n < 4; ++n)
+              a[n] = pack_bf16x2(__uint_as_float(r[4 * (4 * mm + n) + 2 * rs]) * inv,
+                                 __uint_as_float(r[4 * (4 * mm + n) + 2 * rs + 1]) * inv);
+            quad_transpose4(a, fc);
+            if (ok)
+              *reinterpret_cast<uint4 *>(reinterpret_cast<__nv_bfloat16 *>(base) + (size_t)lr * stride + col) =
+                  make_uint4(a[0], a[1], a[2], a[3]);
+          } else {
+            uint32_t lo[4], hi[4];
+#pragma unroll
+            for (int n = 0; n < 4; ++n) {
+              lo[n] = __float_as_uint(__uint_as_float(r[4 * (4 * mm + n) + 2 * rs]) * inv);
+              hi[n] = __float_as_uint(__uint_as_float(r[4 * (4 * mm + n) + 2 * rs + 1]) * inv);
+            }
+            quad_transpose4(lo, fc);
+            quad_transpose4(hi, fc);
+            if (ok) {
+              uint4 *d = reinterpret_cast<uint4 *>(reinterpret_cast<float *>(base) + (size_t)lr * stride + col);
+              d[0] = make_uint4(lo[0], hi[0], lo[1], hi[1]);
+              d[1] = make_uint4(lo[2], hi[2], lo[3], hi[3]);
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
 } // namespace
 
 // kTrace (instantiated in -DSLACK_DIAGNOSTICS builds only): records clock64() time stamps of CTA 0's first item into p.dbg_t (slack_debug_set key 1):
@@ -565,16 +621,35 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
     [[maybe_unused]] uint32_t ring = 0; // FP8: ring entry of the item's first K tile (the producer's count; scale slots)
     bool first_item = true;
     int adv = 1;
+    // The queue's records are read one item AHEAD (the loads of the next one are issued before the epilogue and land while
+    // it runs): two dependent global loads at the top of every item cost the softmax warps ~4000 cycles per item.
+    DevItem it0 = p.items[min(item_begin, max(item_end - 1, item_begin))];
+    [[maybe_unused]] DevItem it1 = it0; // dual kernels: the record behind it0 (the companion of a dual item)
+    if constexpr (kDualOk) it1 = p.items[min(item_begin + 1, max(item_end - 1, item_begin))];
+    DevItem nx0 = it0;
+    [[maybe_unused]] DevItem nx1 = it0;
     for (int k = item_begin; k < item_end; k += adv) {
       // dual item: tile slot 1 serves the queue's NEXT item (its own rows 0.., head, mask columns, output rows)
-      const bool dual = kDualOk && p.items[k].dual != 0;
+      const bool dual = kDualOk && it0.dual != 0;
       adv = dual ? 2 : 1;
-      const DevItem it = p.items[k + ((dual && i == 1) ? 1 : 0)];
+      const DevItem it = (dual && i == 1) ? it1 : it0;
+      auto load_next = [&]() {
+        nx0 = p.items[min(k + adv, item_end - 1)];
+        if constexpr (kDualOk) nx1 = p.items[min(k + adv + 1, item_end - 1)];
+      };
+      auto rotate = [&]() {
+        it0 = nx0;
+        if constexpr (kDualOk) it1 = nx1;
+      };
       const ItemView v = view_of(it);
       const int row_base = dual ? 0 : i * kTileM; // this tile's first row inside ITS item
       [[maybe_unused]] const uint32_t r0 = ring;
       if constexpr (kFp8) ring += (dual ? 4u : 2u) * (uint32_t)v.T; // every role counts the tiles, also the one that skips the item
-      if (!dual && i >= v.nq) continue;
+      if (!dual && i >= v.nq) {
+        load_next();
+        rotate();
+        continue;
+      }
       const int Ts = kSparse ? p.item_steps[k] : v.T;
       const uint16_t *steps = kSparse ? p.steps + it.step_off : nullptr;
       if (Ts == 0) { // block-sparse: no selected key tile in this item: out = 0, lse = -inf; no barrier is touched
@@ -593,6 +668,8 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
             p.ws_lse[(size_t)it.partial_slot * kItemRows + local_row] = -INFINITY;
           }
         }
+        load_next();
+        rotate();
         continue;
       }
       float m = -INFINITY, l = 0.f;
@@ -762,57 +839,26 @@ attn_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap tm_q, const
         ++cnt;
       }
       // ---------------- epilogue: O / l ----------------
+      load_next();
       mbar_wait(bar(BAR_O_FINAL + i), itn & 1u, 310 + i, dbg);
       tc_fence_after();
       const float inv_l = kFp8 ? 0.0078125f / l : 1.0f / l; // FP8: O was accumulated from P = 128 * probabilities
       const int local_row = row_base + row;
       const bool valid = local_row < it.q_rows;
       const float lse_val = ((kFp8 ? m : m * sl2) + log2f(l)) * kLn2;
-      if (it.partial_slot < 0) {
-        __nv_bfloat16 *dst =
-            reinterpret_cast<__nv_bfloat16 *>(p.out) + ((size_t)(it.q_row0 + local_row) * H + it.head) * kD;
-#pragma unroll
-        for (int c = 0; c < kD / 32; ++c) {
-          uint32_t r[32];
-          tmem_ld32(tO + (uint32_t)(c * 32), r);
-          tmem_wait_ld();
-          if (valid) {
-#pragma unroll
-            for (int e = 0; e < 32; e += 8) {
-              uint4 o;
-              o.x = pack_bf16x2(__uint_as_float(r[e + 0]) * inv_l, __uint_as_float(r[e + 1]) * inv_l);
-              o.y = pack_bf16x2(__uint_as_float(r[e + 2]) * inv_l, __uint_as_float(r[e + 3]) * inv_l);
-              o.z = pack_bf16x2(__uint_as_float(r[e + 4]) * inv_l, __uint_as_float(r[e + 5]) * inv_l);
-              o.w = pack_bf16x2(__uint_as_float(r[e + 6]) * inv_l, __uint_as_float(r[e + 7]) * inv_l);
-              *reinterpret_cast<uint4 *>(dst + c * 32 + e) = o;
-            }
-          }
-        }
-        if (valid && p.lse != nullptr) p.lse[(size_t)it.head * p.total_q + it.q_row0 + local_row] = lse_val;
-      } else {
-        float *dst = p.ws_o + ((size_t)it.partial_slot * kItemRows + local_row) * kD;
-#pragma unroll
-        for (int c = 0; c < kD / 32; ++c) {
-          uint32_t r[32];
-          tmem_ld32(tO + (uint32_t)(c * 32), r);
-          tmem_wait_ld();
-          if (valid) {
-#pragma unroll
-            for (int e = 0; e < 32; e += 4) {
-              float4 o;
-              o.x = __uint_as_float(r[e + 0]) * inv_l;
-              o.y = __uint_as_float(r[e + 1]) * inv_l;
-              o.z = __uint_as_float(r[e + 2]) * inv_l;
-              o.w = __uint_as_float(r[e + 3]) * inv_l;
-              *reinterpret_cast<float4 *>(dst + c * 32 + e) = o;
-            }
-          }
-        }
-        if (valid) p.ws_lse[(size_t)it.partial_slot * kItemRows + local_row] = lse_val;
+      store_o<kD>(tO, inv_l, lane, row_base + w4 * 32, it.q_rows, it.partial_slot < 0,
+                  it.partial_slot < 0
+                      ? static_cast<void *>(reinterpret_cast<__nv_bfloat16 *>(p.out) + ((size_t)it.q_row0 * H + it.head) * kD)
+                      : static_cast<void *>(p.ws_o + (size_t)it.partial_slot * kItemRows * kD),
+                  it.partial_slot < 0 ? (size_t)H * kD : (size_t)kD);
+      if (valid) {
+        if (it.partial_slot >= 0) p.ws_lse[(size_t)it.partial_slot * kItemRows + local_row] = lse_val;
+        else if (p.lse != nullptr) p.lse[(size_t)it.head * p.total_q + it.q_row0 + local_row] = lse_val;
       }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(BAR_O_FREE + i));
+      rotate();
       ++itn;
       first_item = false;
     }

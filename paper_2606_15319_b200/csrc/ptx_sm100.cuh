@@ -180,6 +180,37 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
       : "r"(taddr)
       : "memory");
 }
+// 16 lanes x 256 bit, 8 repetitions = 64 columns of 16 TMEM lanes starting at the lane of `taddr` (the warp's lane quadrant
+// base, or that + 16).  Fragment layout (as the mma m16n8 accumulator): with g = lane / 4, c = lane % 4, repetition n holds
+// r[4n], r[4n+1] = row g, columns 8n + 2c, + 1 and r[4n+2], r[4n+3] = row g + 8, same columns: a quad of lanes owns 8
+// consecutive columns of a row, which is what lets the epilogue write rows in 64-byte runs.
+__device__ __forceinline__ void tmem_ld_16x256b_x8(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.16x256b.x8.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr)
+      : "memory");
+}
+// 4 x 4 transpose of 32-bit words inside every quad of lanes: on return a[j] of lane c (= lane % 4) is what a[c] of lane
+// (lane - c + j) held.  Two butterfly stages, 4 shuffles.
+__device__ __forceinline__ void quad_transpose4(uint32_t (&a)[4], int c) {
+  const bool odd = c & 1, hi = c & 2;
+  uint32_t x = odd ? a[0] : a[1], y = odd ? a[2] : a[3];
+  x = __shfl_xor_sync(0xffffffffu, x, 1);
+  y = __shfl_xor_sync(0xffffffffu, y, 1);
+  if (odd) a[0] = x, a[2] = y;
+  else a[1] = x, a[3] = y;
+  x = hi ? a[0] : a[2], y = hi ? a[1] : a[3];
+  x = __shfl_xor_sync(0xffffffffu, x, 2);
+  y = __shfl_xor_sync(0xffffffffu, y, 2);
+  if (hi) a[0] = x, a[1] = y;
+  else a[2] = x, a[3] = y;
+}
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
   asm volatile(
       "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
