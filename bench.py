@@ -266,7 +266,7 @@ def run_reference(args):
 # of that workload (ncu cannot run inside a timed bench; profiles/ names the command): null where none was taken.
 NCU_TRAFFIC_BYTES = {
     "cfg2": (216167680, "profiles/r01_ncu_full_cfg2.md"),
-    "cfg5": (1026880768, "profiles/r02_ncu_full_cfg5_final.md"),   # Lk = 32760 only
+    "cfg5": (1038073088, "profiles/r02_ncu_full_cfg5_final.md"),   # Lk = 32760 only
 }
 
 
